@@ -1,0 +1,164 @@
+/* include/lbm.h — C ABI of liblbm_b200.so: the per-time-step update of the 2-D (D2Q9) color-gradient
+ * lattice Boltzmann model with the ghost-node wetting boundary condition of arxiv/paper_2605_30878,
+ * hand-written CUDA for sm_100a (B200).  One GPU, fp64 or fp32 device arithmetic.
+ *
+ * What the calls compute (citations are PAPER.md lines; "R<k>" are the readings in DESIGN.md):
+ *   lbm_create   node classes (a fluid/solid boundary node has >= 1 solid/fluid D2Q9
+ *                neighbour), the index-sorted ghost-node list with analytic unit normals n_s
+ *                (:100), the point x_F = x_G + dx n_s and its bilinear stencil (:66, Fig. 2).
+ *   lbm_init     phi on solid nodes = (1 + cos theta)/2 (:100); N_i = N_i^eq(p = 0, u0) (Eq. A4,
+ *                :275), B_i = phi N_i (R14); first ghost update (Eq. 9, :78-80).
+ *   lbm_step     n x { collision A1 (:264) with velocity-based equilibrium A4, forcing A8-A11
+ *                (:290-302), surface tension Eq. 4 (:45), segregation A12 (:307); propagation
+ *                A16-A17 (:318-322) with half-way bounce-back (R12); phi = sum_i B_i (A13, :311);
+ *                ghost update phi_G = phi_F / (phi_F + (1 - phi_F) e^eps), eps = -4 dx cos(theta)/W
+ *                (Eq. 9, :78-80) }.
+ *   lbm_get      rho (:43), phi (A13), u (A14, :313), p (A15, :315) at the current time.
+ *
+ * Conventions: node (i, j) sits at (x, y) = (i, j); linear index idx = j*nx + i (x fastest);
+ * periodic in both directions; flat walls are rows of solid nodes inside the array; dx = dt = 1;
+ * c_s^2 = 1/3; direction order of Eq. A5 (:280):
+ *   c = (0,0),(1,0),(0,1),(-1,0),(0,-1),(1,1),(-1,1),(-1,-1),(1,-1).
+ * Population arrays are structure-of-arrays: pop[q*nx*ny + idx].
+ *
+ * Memory and ownership: every pointer is the caller's.  Pointers marked HOST must be host
+ * memory (pageable or pinned) and are only used during the call; they are never retained.
+ * `d_workspace` (DEVICE) is the only device memory the context uses for its state; it must stay
+ * allocated until lbm_destroy and be at least `workspace_bytes` (from lbm_plan) long, 256-byte
+ * aligned.  `cuda_stream` is a borrowed cudaStream_t (0 = default stream); all work of a context
+ * is enqueued on it.  A context is not thread-safe; different contexts are independent.
+ *
+ * Errors: every int-returning call returns LBM_OK (0) or a negative code; nothing throws or aborts
+ * across the ABI; lbm_last_error(ctx) holds a readable message (for LBM_ECUDA the CUDA error
+ * string).  There is NO CPU fallback: without a usable CUDA device every compute call fails with
+ * LBM_ECUDA.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3 };
+
+/* node classes (Fig. 1) */
+enum { LBM_FLUID_BULK = 0, LBM_FLUID_BOUNDARY = 1, LBM_GHOST = 2, LBM_SOLID_BULK = 3 };
+
+/* launch schedules of lbm_step (same arithmetic per node, different kernel decomposition) */
+enum {
+  LBM_SCHEDULE_AUTO = 0,      /* the fastest schedule available (currently FUSED)                 */
+  LBM_SCHEDULE_BASELINE = 1,  /* 3 launches/step: collide+stream, phi = sum B, ghost; N and B in HBM */
+  LBM_SCHEDULE_FUSED = 2      /* 2 launches/step: tiled collide+stream that also produces phi(t+1)
+                                 from B* held in shared memory (B never touches HBM), ghost        */
+};
+
+typedef struct lbm_ctx lbm_ctx;                 /* opaque; one simulation                         */
+
+typedef struct { double cx, cy, r; } lbm_disk;  /* analytic solid: closed disk, periodic images   */
+
+typedef struct {
+  int32_t nx, ny;          /* grid; both >= 3                                                     */
+  int32_t precision;       /* 64 or 32: device storage and arithmetic (host I/O is always double) */
+  int32_t wall_rows;       /* 1: rows j = 0 and j = ny-1 are flat walls (must be solid in mask)   */
+  int32_t ghost_rule;      /* 0: Eq. 9 (the paper's rule); 1: Eq. 10 (Fakhari-Bolster, :84)       */
+  int32_t schedule;        /* LBM_SCHEDULE_*                                                      */
+  double  rho_l, rho_g;    /* phase densities (:43); "density ratio" = rho_l / rho_g              */
+  double  nu_l, nu_g;      /* kinematic viscosities; tau = 1/2 + 3 nu (:273)                      */
+  double  sigma, W;        /* surface tension, interface width (Eq. 4-5); W >= 4 (:80)            */
+  double  theta_deg;       /* equilibrium contact angle measured in the liquid (:60), [0, 180]    */
+  double  mobility;        /* M_phi at reference p = 0: alpha = 1 - 10 M_phi / 3 (:288, R5)       */
+  double  gx, gy;          /* body acceleration, F_b = rho g (Eq. 2, :39)                         */
+} lbm_params;
+
+/* Sizes a context.  mask: HOST, nx*ny bytes, non-zero = solid.  Runs the classification kernel
+ * once on a temporary device copy of the mask (cudaMalloc/cudaFree inside the call) and returns
+ * the exact number of ghost nodes and the workspace size lbm_create needs.  Either output may be
+ * NULL.  LBM_EINVAL on bad parameters (sizes < 3, rho <= 0, nu <= 0, W < 4, sigma < 0, theta
+ * outside [0,180], mobility outside (0, 0.3), precision not 32/64, wall rows not solid). */
+int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_t* workspace_bytes);
+
+/* Builds a context in the caller's device workspace.  mask: HOST nx*ny bytes (copied).
+ * disks: HOST array of n_disks analytic disks whose rasterisation produced the solid nodes of the
+ * mask (closed disks, minimum-image distance^2 <= r^2); every ghost node that is not on a wall
+ * row must lie in at least one disk, else LBM_EINVAL ("mask and geometry disagree").  The owner of
+ * a ghost node is the containing disk with the least depth r - |x_G - x_c| (first wins ties, R17).
+ * LBM_ENOMEM if workspace_bytes is too small. */
+int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const lbm_disk* disks,
+               int32_t n_disks, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Sets the state at time 0.  phi0: HOST nx*ny doubles (values on solid nodes are ignored).
+ * u0: HOST 2*nx*ny doubles (u_x plane then u_y plane) or NULL for a fluid at rest.  Synchronises
+ * the stream before returning. */
+int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0);
+
+/* Advances n >= 0 time steps.  Asynchronous: kernels are enqueued on the stream. */
+int lbm_step(lbm_ctx* ctx, int64_t n);
+
+/* Blocks until all enqueued work of the context has finished. */
+int lbm_sync(lbm_ctx* ctx);
+
+/* Macroscopic fields at the current time, HOST nx*ny doubles each, any may be NULL.  phi carries
+ * this time's ghost values on ghost nodes and (1+cos theta)/2 on bulk solid nodes; rho = u = p = 0
+ * on solid nodes ("fluid dynamical quantities are not evaluated at these nodes", :21).  p is the
+ * auxiliary pressure of Eq. A15 (p_h = rho p).  Synchronises. */
+int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, double* p);
+
+/* Post-stream populations N_i(x, t), B_i(x, t) of the current time, HOST 9*nx*ny doubles each
+ * (SoA), either may be NULL; zeros on solid nodes.  Under LBM_SCHEDULE_FUSED the B_i are not part
+ * of the stored state: they are available right after lbm_init, and after lbm_step only if
+ * lbm_keep_B(ctx, 1) was set before that step (else LBM_EINVAL for B != NULL).  Synchronises. */
+int lbm_get_populations(lbm_ctx* ctx, double* N, double* B);
+
+/* FUSED schedule only: when on != 0 the last time step of every lbm_step call also writes the
+ * post-collision B_i* to HBM (workspace is sized for it) so that lbm_get_populations can return
+ * B_i.  No effect on the arithmetic.  Ignored by the BASELINE schedule (B always stored). */
+int lbm_keep_B(lbm_ctx* ctx, int32_t on);
+
+/* Populations at selected nodes only (for parity checks at sizes where 18 full arrays are too
+ * much to move): idx HOST n_idx int64 node indices; N, B HOST 9*n_idx doubles (q-major:
+ * out[q*n_idx + k]); B may be NULL (same availability rule as lbm_get_populations). */
+int lbm_sample_populations(lbm_ctx* ctx, int64_t n_idx, const int64_t* idx, double* N, double* B);
+
+/* Classification and ghost geometry (all HOST, any may be NULL): cls nx*ny bytes (LBM_* classes);
+ * *n_ghost; then per ghost node in increasing idx: ghost_idx[n_ghost], unit normal
+ * (ghost_nx, ghost_ny), depth below the surface, the 4 bilinear corner indices ghost_corner
+ * [4*n_ghost] and weights ghost_wgt[4*n_ghost] of x_F (order (i0,j0),(i0+1,j0),(i0,j0+1),
+ * (i0+1,j0+1)). */
+int lbm_get_classification(lbm_ctx* ctx, uint8_t* cls, int32_t* n_ghost, int32_t* ghost_idx,
+                           double* ghost_nx, double* ghost_ny, double* ghost_depth,
+                           int32_t* ghost_corner, double* ghost_wgt);
+
+/* Diagnostics over fluid nodes at the current time (warp-shuffle + fixed-tree block reductions,
+ * deterministic): out[0] = sum phi, [1] = sum (1 - phi), [2] = 1/2 sum rho |u|^2, [3] = max |u|,
+ * [4] = min phi, [5] = max phi, [6] = number of fluid nodes, [7] = 1 if any NaN.  out: HOST. */
+int lbm_diag(lbm_ctx* ctx, double out[8]);
+
+/* Test hook: the local update of `count` independent nodes on the device, in the context-free
+ * precision `precision` (32/64).  N: HOST 9*count doubles (node-major: N[9*k + q]), phi_nb: HOST
+ * 9*count doubles, phi_nb[9*k + q] = phi(x + c_q); outputs Nstar, Bstar (9*count) and fields
+ * (8*count: rho, tau, ux, uy, p, Fx, Fy, |grad phi|), any may be NULL. */
+int lbm_node_update_batch(const lbm_params* prm, int64_t count, const double* N,
+                          const double* phi_nb, double* Nstar, double* Bstar, double* fields);
+
+/* Measurement helper: advances n steps like lbm_step but brackets every kernel launch with CUDA
+ * events on the context's stream and returns, after synchronising, the summed device time in
+ * milliseconds per kernel kind: ms[0] = collide(+stream), ms[1] = phi-sum (BASELINE only),
+ * ms[2] = ghost update.  The event records add a little launch overhead; use lbm_step for
+ * throughput and this call for the per-kernel split. */
+int lbm_step_timed(lbm_ctx* ctx, int64_t n, double ms[3]);
+
+/* Device-timing helper: per-kernel-kind accumulated launch counts since the last reset;
+ * counts[0] = collide(+stream), [1] = phi-sum, [2] = ghost, [3] = other. */
+int lbm_launch_counts(lbm_ctx* ctx, int64_t counts[4], int32_t reset);
+
+const char* lbm_last_error(const lbm_ctx* ctx); /* ctx may be NULL: last error of lbm_plan/create */
+const char* lbm_version(void);
+void lbm_destroy(lbm_ctx* ctx);                 /* frees the host handle only; workspace is the caller's */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,607 @@
+// lbm_api.cu — host side of liblbm_b200.so: the C ABI of include/lbm.h, workspace carving and
+// the launch schedule.  No CPU fallback: every compute call needs a CUDA device.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/lbm.h"
+#include "lbm_fused.cuh"
+#include "lbm_kernels.cuh"
+
+using namespace lbm;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+struct Arena {  // carves 256-byte aligned chunks out of the caller's workspace
+  char* base;
+  size_t off;
+  template <typename T>
+  T* take(size_t count) {
+    off = (off + 255) & ~(size_t)255;
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += count * sizeof(T);
+    return p;
+  }
+};
+
+}  // namespace
+
+struct lbm_ctx {
+  lbm_params P;
+  size_t n;
+  int ng;
+  int is32;
+  int fused;
+  int keep_B;
+  int B_valid;       // B planes of buffer `cur` hold the post-collision B* of the last step
+  cudaStream_t st;
+  Consts<double> Cd;
+  Consts<float> Cf;
+  // device arrays (inside the caller's workspace)
+  void* N[2];
+  void* B[2];        // BASELINE: both; FUSED: B[0] only (keep_B / init)
+  void* phi[2];
+  uint8_t* cls;
+  uint8_t* links;
+  int* gidx;
+  int* corner;
+  void* wgt;
+  double* wgt_d;
+  double *gnx, *gny, *gdepth;
+  uint8_t* csolid;
+  int* blk_cnt;
+  int* blk_off;
+  int* scal;          // [0] ghost total, [1] geometry error flag
+  double* stage;      // 5 n doubles (n >= partials)
+  double* diag_out;   // 8 doubles
+  long long* samp_idx;
+  size_t samp_cap;
+  Disk* disks;
+  int n_disks;
+  int cur, pcur;      // population buffer holding the last post-collision state; phi buffer of time t
+  int64_t t;
+  int64_t launches[4];
+  char err[512];
+};
+
+namespace {
+
+int fail(lbm_ctx* c, int code, const char* msg) {
+  snprintf(g_err, sizeof g_err, "%s", msg);
+  if (c) snprintf(c->err, sizeof c->err, "%s", msg);
+  return code;
+}
+
+int cuda_fail(lbm_ctx* c, cudaError_t e, const char* where) {
+  char buf[400];
+  snprintf(buf, sizeof buf, "CUDA error at %s: %s", where, cudaGetErrorString(e));
+  return fail(c, LBM_ECUDA, buf);
+}
+
+#define CK(call)                                                   \
+  do {                                                             \
+    cudaError_t e_ = (call);                                       \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
+  } while (0)
+
+int validate(const lbm_params* P, const char** why) {
+  *why = "";
+  if (!P) { *why = "null params"; return LBM_EINVAL; }
+  if (P->nx < 3 || P->ny < 3) { *why = "nx, ny must be >= 3"; return LBM_EINVAL; }
+  if ((long long)P->nx * P->ny > 0x7fffffffLL / 2) { *why = "nx*ny too large for 32-bit indices"; return LBM_EINVAL; }
+  if (P->precision != 32 && P->precision != 64) { *why = "precision must be 32 or 64"; return LBM_EINVAL; }
+  if (!(P->rho_l > 0.0) || !(P->rho_g > 0.0)) { *why = "densities must be > 0"; return LBM_EINVAL; }
+  if (!(P->nu_l > 0.0) || !(P->nu_g > 0.0)) { *why = "viscosities must be > 0 (tau > 1/2)"; return LBM_EINVAL; }
+  if (!(P->W >= 4.0)) { *why = "W must be >= 4 (PAPER.md:80)"; return LBM_EINVAL; }
+  if (!(P->sigma >= 0.0)) { *why = "sigma must be >= 0"; return LBM_EINVAL; }
+  if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
+  if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
+  if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 2) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
+  return LBM_OK;
+}
+
+int check_walls(const lbm_params* P, const uint8_t* mask) {
+  if (!P->wall_rows) return LBM_OK;
+  for (int i = 0; i < P->nx; i++)
+    if (!mask[i] || !mask[(size_t)(P->ny - 1) * P->nx + i]) return LBM_EINVAL;
+  return LBM_OK;
+}
+
+bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELINE; }
+
+// one layout function serves both sizing (base == nullptr) and carving; everything that does not
+// depend on the ghost count comes first, so a carve with ng = 0 and one with the real ng agree
+// on those arrays
+size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
+  const size_t n = (size_t)P->nx * P->ny;
+  const size_t rs = P->precision == 32 ? 4 : 8;
+  const size_t g = (size_t)(ng > 0 ? ng : 1);
+  const size_t nblk = (n + 255) / 256;
+  const bool fused = use_fused(P);
+  Arena A{base, 0};
+  char* N0 = A.take<char>(9 * n * rs);
+  char* N1 = A.take<char>(9 * n * rs);
+  char* B0 = A.take<char>(9 * n * rs);
+  char* B1 = fused ? nullptr : A.take<char>(9 * n * rs);
+  char* p0 = A.take<char>(n * rs);
+  char* p1 = A.take<char>(n * rs);
+  uint8_t* cls = A.take<uint8_t>(n);
+  uint8_t* links = A.take<uint8_t>(n);
+  int* blk_cnt = A.take<int>(nblk);
+  int* blk_off = A.take<int>(nblk);
+  int* scal = A.take<int>(64);
+  double* stage = A.take<double>(5 * n + 64);
+  double* diag_out = A.take<double>(8);
+  const size_t samp_cap = 1 << 20;
+  long long* samp = A.take<long long>(samp_cap);
+  int* gidx = A.take<int>(g);
+  int* corner = A.take<int>(4 * g);
+  char* wgt = A.take<char>(4 * g * rs);
+  double* wgt_d = A.take<double>(4 * g);
+  double* gnx = A.take<double>(g);
+  double* gny = A.take<double>(g);
+  double* gdepth = A.take<double>(g);
+  uint8_t* csolid = A.take<uint8_t>(g);
+  if (c && base) {
+    c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
+    c->cls = cls; c->links = links; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
+    c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid; c->blk_cnt = blk_cnt;
+    c->blk_off = blk_off; c->scal = scal; c->stage = stage; c->diag_out = diag_out;
+    c->samp_idx = samp; c->samp_cap = samp_cap;
+  }
+  return ((A.off + 255) & ~(size_t)255) + 256;
+}
+
+template <typename R>
+Consts<R> make_consts(const lbm_params& P) {
+  Consts<R> C;
+  const double alpha = 1.0 - 10.0 * P.mobility / 3.0;   // Eq. A7 text (:288) at reference p = 0 (R5)
+  const double ct = cos(P.theta_deg * M_PI / 180.0);
+  const double eps = -(4.0 / P.W) * ct;                 // Eq. 9 (:80), dx = 1
+  C.nx = P.nx; C.ny = P.ny;
+  C.rho_g = (R)P.rho_g; C.drho = (R)(P.rho_l - P.rho_g);
+  C.inu_g = (R)(1.0 / P.nu_g); C.dinu = (R)(1.0 / P.nu_l - 1.0 / P.nu_g);
+  C.s48W = (R)(P.sigma * 48.0 / P.W); C.s15W = (R)(P.sigma * 1.5 * P.W);
+  C.twoW = (R)(2.0 / P.W);
+  C.gbx = (R)P.gx; C.gby = (R)P.gy;
+  C.chi0 = (R)alpha; C.chi1 = (R)((1.0 - alpha) / 5.0); C.chi5 = (R)((1.0 - alpha) / 20.0);
+  C.E = (R)exp(eps); C.eps = (R)eps;
+  C.phi_solid = (R)(0.5 * (1.0 + ct));
+  C.ghost_rule = P.ghost_rule;
+  return C;
+}
+
+dim3 row_grid(int nx, int ny, int* bx) {
+  int b = 256;
+  while (b > 32 && b / 2 >= nx) b /= 2;
+  *bx = b;
+  return dim3((unsigned)((nx + b - 1) / b), (unsigned)ny, 1);
+}
+
+template <typename R> const Consts<R>& consts_of(const lbm_ctx* c);
+template <> const Consts<double>& consts_of<double>(const lbm_ctx* c) { return c->Cd; }
+template <> const Consts<float>& consts_of<float>(const lbm_ctx* c) { return c->Cf; }
+
+// phi(t) fluid part is in phi[pcur]; finish it with the ghost update
+template <typename R>
+void launch_ghost(lbm_ctx* c) {
+  if (c->ng == 0) return;
+  k_ghost_update<R><<<(c->ng + 127) / 128, 128, 0, c->st>>>(
+      consts_of<R>(c), c->ng, c->gidx, (const int4*)c->corner, (const R*)c->wgt, c->csolid,
+      (const R*)c->phi[c->pcur ^ 1], (R*)c->phi[c->pcur]);
+  c->launches[2]++;
+}
+
+struct StepTimer {   // optional event brackets around each launch (lbm_step_timed)
+  cudaEvent_t ev[4];
+  double ms[3];
+};
+
+template <typename R>
+int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
+  int bx;
+  if (tm) cudaEventRecord(tm->ev[0], c->st);
+  const dim3 grid = row_grid(c->P.nx, c->P.ny, &bx);
+  const Consts<R>& C = consts_of<R>(c);
+  if (!c->fused) {
+    k_collide_baseline<R><<<grid, bx, 0, c->st>>>(C, c->cls, c->links, (const R*)c->N[c->cur],
+                                                 (R*)c->N[c->cur ^ 1], (R*)c->B[c->cur ^ 1],
+                                                 (const R*)c->phi[c->pcur]);
+    c->cur ^= 1;
+    c->pcur ^= 1;
+    if (tm) cudaEventRecord(tm->ev[1], c->st);
+    k_phi_sum<R><<<grid, bx, 0, c->st>>>(C, c->cls, c->links, (const R*)c->B[c->cur], (R*)c->phi[c->pcur]);
+    c->launches[0]++;
+    c->launches[1]++;
+    c->B_valid = 1;
+  } else {
+    launch_fused_step<R>(C, c->cls, c->links, (const R*)c->N[c->cur], (R*)c->N[c->cur ^ 1],
+                         write_B ? (R*)c->B[0] : nullptr, (const R*)c->phi[c->pcur],
+                         (R*)c->phi[c->pcur ^ 1], c->st);
+    c->cur ^= 1;
+    c->pcur ^= 1;
+    c->launches[0]++;
+    c->B_valid = write_B ? 1 : 0;
+    if (tm) cudaEventRecord(tm->ev[1], c->st);
+  }
+  if (tm) cudaEventRecord(tm->ev[2], c->st);
+  launch_ghost<R>(c);
+  c->t++;
+  if (tm) {
+    cudaEventRecord(tm->ev[3], c->st);
+    cudaEventSynchronize(tm->ev[3]);
+    float a = 0, b = 0, g = 0;
+    cudaEventElapsedTime(&a, tm->ev[0], tm->ev[1]);
+    cudaEventElapsedTime(&b, tm->ev[1], tm->ev[2]);
+    cudaEventElapsedTime(&g, tm->ev[2], tm->ev[3]);
+    tm->ms[0] += a; tm->ms[1] += b; tm->ms[2] += g;
+  }
+  return LBM_OK;
+}
+
+const void* B_planes(const lbm_ctx* c) { return c->fused ? c->B[0] : c->B[c->cur]; }
+
+}  // namespace
+
+extern "C" {
+
+const char* lbm_version(void) { return "liblbm_b200 0.1 (sm_100a)"; }
+
+const char* lbm_last_error(const lbm_ctx* ctx) { return ctx ? ctx->err : g_err; }
+
+int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_t* workspace_bytes) {
+  lbm_ctx* ctx = nullptr;
+  const char* why;
+  if (validate(prm, &why) != LBM_OK) return fail(nullptr, LBM_EINVAL, why);
+  if (!mask) return fail(nullptr, LBM_EINVAL, "null mask");
+  if (check_walls(prm, mask) != LBM_OK) return fail(nullptr, LBM_EINVAL, "wall rows are not solid in the mask");
+  const size_t n = (size_t)prm->nx * prm->ny;
+  uint8_t* d_mask = nullptr;
+  unsigned long long* d_tot = nullptr;
+  CK(cudaMalloc(&d_mask, n + 8));
+  cudaError_t e = cudaMalloc(&d_tot, 8);
+  if (e != cudaSuccess) { cudaFree(d_mask); return cuda_fail(nullptr, e, "cudaMalloc"); }
+  unsigned long long tot = 0;
+  e = cudaMemcpy(d_mask, mask, n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemset(d_tot, 0, 8);
+  if (e == cudaSuccess) {
+    k_classify<<<(unsigned)((n + 255) / 256), 256>>>(d_mask, prm->nx, prm->ny, nullptr, nullptr, nullptr, d_tot);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(&tot, d_tot, 8, cudaMemcpyDeviceToHost);
+  cudaFree(d_mask);
+  cudaFree(d_tot);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "lbm_plan");
+  if (n_ghost) *n_ghost = (int64_t)tot;
+  if (workspace_bytes) *workspace_bytes = layout(nullptr, nullptr, prm, (long long)tot);
+  return LBM_OK;
+}
+
+int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const lbm_disk* disks,
+               int32_t n_disks, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  lbm_ctx* ctx = nullptr;
+  if (!out) return fail(nullptr, LBM_EINVAL, "null out");
+  *out = nullptr;
+  const char* why;
+  if (validate(prm, &why) != LBM_OK) return fail(nullptr, LBM_EINVAL, why);
+  if (!mask) return fail(nullptr, LBM_EINVAL, "null mask");
+  if (n_disks < 0 || (n_disks > 0 && !disks)) return fail(nullptr, LBM_EINVAL, "bad disk list");
+  if (check_walls(prm, mask) != LBM_OK) return fail(nullptr, LBM_EINVAL, "wall rows are not solid in the mask");
+  if (!d_workspace || ((uintptr_t)d_workspace & 255)) return fail(nullptr, LBM_EINVAL, "workspace null or not 256-byte aligned");
+  const size_t n = (size_t)prm->nx * prm->ny;
+  // the disk list and the mask upload need room before the ghost count is known
+  const size_t min_ws = layout(nullptr, nullptr, prm, 0);
+  if (workspace_bytes < min_ws) return fail(nullptr, LBM_ENOMEM, "workspace too small");
+
+  lbm_ctx* c = new (std::nothrow) lbm_ctx;
+  if (!c) return fail(nullptr, LBM_ENOMEM, "host allocation failed");
+  memset(c, 0, sizeof *c);
+  ctx = c;
+  c->P = *prm;
+  c->n = n;
+  c->is32 = prm->precision == 32;
+  c->fused = use_fused(prm) ? 1 : 0;
+  c->st = (cudaStream_t)cuda_stream;
+  c->Cd = make_consts<double>(*prm);
+  c->Cf = make_consts<float>(*prm);
+  layout(c, (char*)d_workspace, prm, 0);   // provisional carve: cls/links/blk arrays do not depend on ng
+
+#define CKC(call)                                                              \
+  do {                                                                         \
+    cudaError_t e_ = (call);                                                   \
+    if (e_ != cudaSuccess) { int rc_ = cuda_fail(nullptr, e_, #call); delete c; return rc_; } \
+  } while (0)
+
+  // (1) classification; the mask is staged in the (not yet used) stage area
+  uint8_t* d_mask = reinterpret_cast<uint8_t*>(c->stage);
+  const unsigned nblk = (unsigned)((n + 255) / 256);
+  CKC(cudaMemcpyAsync(d_mask, mask, n, cudaMemcpyHostToDevice, c->st));
+  k_classify<<<nblk, 256, 0, c->st>>>(d_mask, prm->nx, prm->ny, c->cls, c->links, c->blk_cnt, nullptr);
+  k_scan_blocks<<<1, 1024, 0, c->st>>>(c->blk_cnt, (int)nblk, c->blk_off, c->scal);
+  CKC(cudaGetLastError());
+  int ng = 0;
+  CKC(cudaMemcpyAsync(&ng, c->scal, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+  CKC(cudaStreamSynchronize(c->st));
+  c->ng = ng;
+  const size_t need = layout(nullptr, nullptr, prm, ng);
+  if (workspace_bytes < need) {
+    delete c;
+    return fail(nullptr, LBM_ENOMEM, "workspace too small for the ghost list (size it with lbm_plan)");
+  }
+  layout(c, (char*)d_workspace, prm, ng);   // ghost arrays now have their real extent
+
+  // (2) index-sorted ghost list and per-ghost geometry
+  if (ng > 0) {
+    k_compact_ghosts<<<nblk, 256, 0, c->st>>>(c->cls, (long long)n, c->blk_off, c->gidx);
+    // disk list staged behind the mask copy in the stage area (5n doubles >= n bytes + disks?)
+    const size_t disk_bytes = (size_t)n_disks * sizeof(Disk);
+    const size_t stage_bytes = (5 * n + 64) * sizeof(double);
+    const size_t disk_off = (n + 255) & ~(size_t)255;
+    if (disk_off + disk_bytes > stage_bytes) {
+      delete c;
+      return fail(nullptr, LBM_EINVAL, "too many disks for this grid");
+    }
+    Disk* d_disks = reinterpret_cast<Disk*>(reinterpret_cast<char*>(c->stage) + disk_off);
+    static_assert(sizeof(Disk) == sizeof(lbm_disk), "disk layout");
+    if (n_disks > 0) CKC(cudaMemcpyAsync(d_disks, disks, disk_bytes, cudaMemcpyHostToDevice, c->st));
+    CKC(cudaMemsetAsync(c->scal + 1, 0, sizeof(int), c->st));
+    const unsigned gb = (unsigned)((ng + 127) / 128);
+    if (c->is32)
+      k_ghost_geometry<float><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
+                                                     n_disks, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
+                                                     c->wgt_d, (float*)c->wgt, c->csolid, c->scal + 1);
+    else
+      k_ghost_geometry<double><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
+                                                      n_disks, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
+                                                      c->wgt_d, (double*)c->wgt, c->csolid, c->scal + 1);
+    CKC(cudaGetLastError());
+    int bad = 0;
+    CKC(cudaMemcpyAsync(&bad, c->scal + 1, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CKC(cudaStreamSynchronize(c->st));
+    if (bad) {
+      delete c;
+      return fail(nullptr, LBM_EINVAL, "mask and geometry disagree: a ghost node lies in no disk");
+    }
+  }
+  CKC(cudaStreamSynchronize(c->st));
+#undef CKC
+  *out = c;
+  return LBM_OK;
+}
+
+void lbm_destroy(lbm_ctx* ctx) { delete ctx; }
+
+int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
+  if (!ctx || !phi0) return fail(ctx, LBM_EINVAL, "null argument");
+  const size_t n = ctx->n;
+  double* d_phi0 = ctx->stage;
+  double* d_u0 = u0 ? ctx->stage + n : nullptr;
+  CK(cudaMemcpyAsync(d_phi0, phi0, n * sizeof(double), cudaMemcpyHostToDevice, ctx->st));
+  if (u0) CK(cudaMemcpyAsync(d_u0, u0, 2 * n * sizeof(double), cudaMemcpyHostToDevice, ctx->st));
+  ctx->cur = 0;
+  ctx->pcur = 0;
+  ctx->t = 0;
+  int bx;
+  const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];
+  if (ctx->is32)
+    k_init<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, d_phi0, d_u0, (float*)ctx->N[0],
+                                            (float*)Bp, (float*)ctx->phi[0], (float*)ctx->phi[1]);
+  else
+    k_init<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, d_phi0, d_u0, (double*)ctx->N[0],
+                                             (double*)Bp, (double*)ctx->phi[0], (double*)ctx->phi[1]);
+  ctx->launches[3]++;
+  ctx->B_valid = 1;
+  if (ctx->is32) launch_ghost<float>(ctx); else launch_ghost<double>(ctx);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(ctx->st));
+  return LBM_OK;
+}
+
+int lbm_step(lbm_ctx* ctx, int64_t nsteps) {
+  if (!ctx || nsteps < 0) return fail(ctx, LBM_EINVAL, "bad argument");
+  for (int64_t s = 0; s < nsteps; s++) {
+    const bool wb = ctx->fused && ctx->keep_B && s == nsteps - 1;
+    if (ctx->is32) step_once<float>(ctx, wb); else step_once<double>(ctx, wb);
+  }
+  CK(cudaGetLastError());
+  return LBM_OK;
+}
+
+int lbm_step_timed(lbm_ctx* ctx, int64_t nsteps, double ms[3]) {
+  if (!ctx || nsteps < 0 || !ms) return fail(ctx, LBM_EINVAL, "bad argument");
+  StepTimer tm;
+  tm.ms[0] = tm.ms[1] = tm.ms[2] = 0.0;
+  for (int k = 0; k < 4; k++) CK(cudaEventCreate(&tm.ev[k]));
+  CK(cudaStreamSynchronize(ctx->st));
+  for (int64_t s = 0; s < nsteps; s++) {
+    const bool wb = ctx->fused && ctx->keep_B && s == nsteps - 1;
+    if (ctx->is32) step_once<float>(ctx, wb, &tm); else step_once<double>(ctx, wb, &tm);
+  }
+  for (int k = 0; k < 4; k++) cudaEventDestroy(tm.ev[k]);
+  CK(cudaGetLastError());
+  for (int k = 0; k < 3; k++) ms[k] = tm.ms[k];
+  return LBM_OK;
+}
+
+int lbm_sync(lbm_ctx* ctx) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  CK(cudaStreamSynchronize(ctx->st));
+  return LBM_OK;
+}
+
+int lbm_keep_B(lbm_ctx* ctx, int32_t on) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  ctx->keep_B = on ? 1 : 0;
+  return LBM_OK;
+}
+
+int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, double* p) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  const size_t n = ctx->n;
+  double* s = ctx->stage;
+  double* d[5] = {rho ? s : nullptr, phi ? s + n : nullptr, ux ? s + 2 * n : nullptr,
+                  uy ? s + 3 * n : nullptr, p ? s + 4 * n : nullptr};
+  double* h[5] = {rho, phi, ux, uy, p};
+  int bx;
+  const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  if (ctx->is32)
+    k_moments<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)ctx->N[ctx->cur],
+                                               (const float*)ctx->phi[ctx->pcur], d[0], d[1], d[2], d[3], d[4]);
+  else
+    k_moments<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)ctx->N[ctx->cur],
+                                                (const double*)ctx->phi[ctx->pcur], d[0], d[1], d[2], d[3], d[4]);
+  ctx->launches[3]++;
+  CK(cudaGetLastError());
+  for (int f = 0; f < 5; f++)
+    if (h[f]) CK(cudaMemcpyAsync(h[f], d[f], n * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+  CK(cudaStreamSynchronize(ctx->st));
+  return LBM_OK;
+}
+
+int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  if (B && !ctx->B_valid)
+    return fail(ctx, LBM_EINVAL, "B is not stored under the FUSED schedule: call lbm_keep_B(ctx, 1) before lbm_step");
+  const size_t n = ctx->n;
+  int bx;
+  const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  const double chi[9] = {ctx->Cd.chi0, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1,
+                         ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5};
+  for (int which = 0; which < 2; which++) {
+    double* host = which ? B : N;
+    if (!host) continue;
+    const void* pop = which ? B_planes(ctx) : ctx->N[ctx->cur];
+    for (int q0 = 0; q0 < 9; q0 += 5) {          // 5 staging planes at a time
+      const int q1 = q0 + 5 < 9 ? q0 + 5 : 9;
+      for (int q = q0; q < q1; q++) {
+        double* dst = ctx->stage + (size_t)(q - q0) * n;
+        const double add = which ? 0.0 : chi[q];
+        if (ctx->is32)
+          k_gather_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)pop, q, add, dst);
+        else
+          k_gather_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)pop, q, add, dst);
+        ctx->launches[3]++;
+      }
+      CK(cudaGetLastError());
+      CK(cudaMemcpyAsync(host + (size_t)q0 * n, ctx->stage, (size_t)(q1 - q0) * n * sizeof(double),
+                         cudaMemcpyDeviceToHost, ctx->st));
+      CK(cudaStreamSynchronize(ctx->st));
+    }
+  }
+  return LBM_OK;
+}
+
+int lbm_sample_populations(lbm_ctx* ctx, int64_t n_idx, const int64_t* idx, double* N, double* B) {
+  if (!ctx || n_idx < 0 || (n_idx > 0 && !idx)) return fail(ctx, LBM_EINVAL, "bad argument");
+  if (B && !ctx->B_valid)
+    return fail(ctx, LBM_EINVAL, "B is not stored under the FUSED schedule: call lbm_keep_B(ctx, 1) before lbm_step");
+  if ((size_t)n_idx > ctx->samp_cap || (size_t)n_idx * 9 > 5 * ctx->n) return fail(ctx, LBM_EINVAL, "too many samples");
+  for (int64_t t = 0; t < n_idx; t++)
+    if (idx[t] < 0 || (size_t)idx[t] >= ctx->n) return fail(ctx, LBM_EINVAL, "sample index out of range");
+  if (n_idx == 0) return LBM_OK;
+  CK(cudaMemcpyAsync(ctx->samp_idx, idx, (size_t)n_idx * sizeof(long long), cudaMemcpyHostToDevice, ctx->st));
+  const unsigned gb = (unsigned)((n_idx + 127) / 128);
+  for (int which = 0; which < 2; which++) {
+    double* host = which ? B : N;
+    if (!host) continue;
+    const void* pop = which ? B_planes(ctx) : ctx->N[ctx->cur];
+    if (ctx->is32)
+      k_gather_samples<float><<<gb, 128, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)pop, which ? 0 : 1,
+                                                       (long long)n_idx, ctx->samp_idx, ctx->stage);
+    else
+      k_gather_samples<double><<<gb, 128, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)pop, which ? 0 : 1,
+                                                        (long long)n_idx, ctx->samp_idx, ctx->stage);
+    ctx->launches[3]++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(host, ctx->stage, (size_t)n_idx * 9 * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+    CK(cudaStreamSynchronize(ctx->st));
+  }
+  return LBM_OK;
+}
+
+int lbm_get_classification(lbm_ctx* ctx, uint8_t* cls, int32_t* n_ghost, int32_t* ghost_idx,
+                           double* ghost_nx, double* ghost_ny, double* ghost_depth,
+                           int32_t* ghost_corner, double* ghost_wgt) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  const size_t g = (size_t)ctx->ng;
+  if (n_ghost) *n_ghost = ctx->ng;
+  if (cls) CK(cudaMemcpyAsync(cls, ctx->cls, ctx->n, cudaMemcpyDeviceToHost, ctx->st));
+  if (g > 0) {
+    if (ghost_idx) CK(cudaMemcpyAsync(ghost_idx, ctx->gidx, g * sizeof(int), cudaMemcpyDeviceToHost, ctx->st));
+    if (ghost_nx) CK(cudaMemcpyAsync(ghost_nx, ctx->gnx, g * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+    if (ghost_ny) CK(cudaMemcpyAsync(ghost_ny, ctx->gny, g * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+    if (ghost_depth) CK(cudaMemcpyAsync(ghost_depth, ctx->gdepth, g * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+    if (ghost_corner) CK(cudaMemcpyAsync(ghost_corner, ctx->corner, 4 * g * sizeof(int), cudaMemcpyDeviceToHost, ctx->st));
+    if (ghost_wgt) CK(cudaMemcpyAsync(ghost_wgt, ctx->wgt_d, 4 * g * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+  }
+  CK(cudaStreamSynchronize(ctx->st));
+  return LBM_OK;
+}
+
+int lbm_diag(lbm_ctx* ctx, double out[8]) {
+  if (!ctx || !out) return fail(ctx, LBM_EINVAL, "null argument");
+  int bx;
+  const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  const long long m = (long long)grid.x * grid.y;
+  if ((size_t)m * sizeof(DiagVec) > (5 * ctx->n + 64) * sizeof(double)) return fail(ctx, LBM_EINVAL, "grid too small for diag staging");
+  DiagVec* part = reinterpret_cast<DiagVec*>(ctx->stage);
+  if (ctx->is32)
+    k_diag_partial<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)ctx->N[ctx->cur],
+                                                    (const float*)ctx->phi[ctx->pcur], part);
+  else
+    k_diag_partial<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)ctx->N[ctx->cur],
+                                                     (const double*)ctx->phi[ctx->pcur], part);
+  k_diag_final<<<1, 1024, 0, ctx->st>>>(part, m, ctx->diag_out);
+  ctx->launches[3] += 2;
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, ctx->diag_out, 8 * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+  CK(cudaStreamSynchronize(ctx->st));
+  return LBM_OK;
+}
+
+int lbm_launch_counts(lbm_ctx* ctx, int64_t counts[4], int32_t reset) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  if (counts) for (int k = 0; k < 4; k++) counts[k] = ctx->launches[k];
+  if (reset) for (int k = 0; k < 4; k++) ctx->launches[k] = 0;
+  return LBM_OK;
+}
+
+int lbm_node_update_batch(const lbm_params* prm, int64_t count, const double* N, const double* phi_nb,
+                          double* Nstar, double* Bstar, double* fields) {
+  lbm_ctx* ctx = nullptr;
+  const char* why;
+  if (validate(prm, &why) != LBM_OK) return fail(nullptr, LBM_EINVAL, why);
+  if (count < 0 || !N || !phi_nb) return fail(nullptr, LBM_EINVAL, "bad argument");
+  if (count == 0) return LBM_OK;
+  const size_t c9 = (size_t)count * 9 * sizeof(double), c8 = (size_t)count * 8 * sizeof(double);
+  double* d = nullptr;
+  CK(cudaMalloc(&d, 4 * c9 + c8));
+  double *dN = d, *dP = d + 9 * count, *dNs = d + 18 * count, *dBs = d + 27 * count, *dF = d + 36 * count;
+  cudaError_t e = cudaMemcpy(dN, N, c9, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(dP, phi_nb, c9, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    const unsigned gb = (unsigned)((count + 127) / 128);
+    if (prm->precision == 32)
+      k_node_batch<float><<<gb, 128>>>(make_consts<float>(*prm), (long long)count, dN, dP, dNs, dBs, dF);
+    else
+      k_node_batch<double><<<gb, 128>>>(make_consts<double>(*prm), (long long)count, dN, dP, dNs, dBs, dF);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess && Nstar) e = cudaMemcpy(Nstar, dNs, c9, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess && Bstar) e = cudaMemcpy(Bstar, dBs, c9, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess && fields) e = cudaMemcpy(fields, dF, c8, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  cudaFree(d);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "lbm_node_update_batch");
+  return LBM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,574 @@
+// lbm_kernels.cuh — CUDA kernels of liblbm_b200 (sm_100a).  See DESIGN.md "Kernels".
+//
+// State layout in HBM (structure of arrays, x fastest, idx = j*nx + i):
+//   pop[q*n + idx]  post-COLLISION deviations n_q* = N_q* - chi_q of the last step, stored at the
+//                   node that produced them; propagation (A16-A17) is the pull on the next read:
+//                   N_q(x, t+1) = N_q*(x - c_q, t), or N_opp(q)*(x, t) if x - c_q is solid
+//                   (half-way bounce-back, R12).  Double-buffered.
+//   phi[2][idx]     order parameter incl. ghost values, double-buffered so that the ghost update
+//                   is a Jacobi sweep (R13) and tiles may read halos while others write.
+//   cls[idx]        node class (1 byte); links[idx] bounce-back link bits, read only on
+//                   fluid-boundary nodes (bit q-1 set <=> node x - c_q is solid).
+#pragma once
+#include <stdint.h>
+#include "lbm_math.cuh"
+
+namespace lbm {
+
+// opposite direction of Eq. A5's ordering: 1<->3, 2<->4, 5<->7, 6<->8
+__host__ __device__ constexpr int opp(int q) {
+  return q == 0 ? 0 : (q < 5 ? ((q + 1) % 4) + 1 : ((q - 3) % 4) + 5);
+}
+
+// Periodic neighbourhood of node (i, j): linear indices of x - c_q (pull sources) and x + c_q.
+struct Nbr {
+  int src[9];  // idx of x - c_q
+  int dst[9];  // idx of x + c_q
+};
+
+__device__ __forceinline__ Nbr make_nbr(int i, int j, int nx, int ny) {
+  const int im = (i == 0) ? nx - 1 : i - 1, ip = (i == nx - 1) ? 0 : i + 1;
+  const int jm = (j == 0) ? ny - 1 : j - 1, jp = (j == ny - 1) ? 0 : j + 1;
+  const int rm = jm * nx, r0 = j * nx, rp = jp * nx;
+  Nbr b;
+  b.src[0] = r0 + i;  b.dst[0] = r0 + i;
+  b.src[1] = r0 + im; b.dst[1] = r0 + ip;
+  b.src[2] = rm + i;  b.dst[2] = rp + i;
+  b.src[3] = r0 + ip; b.dst[3] = r0 + im;
+  b.src[4] = rp + i;  b.dst[4] = rm + i;
+  b.src[5] = rm + im; b.dst[5] = rp + ip;
+  b.src[6] = rm + ip; b.dst[6] = rp + im;
+  b.src[7] = rp + ip; b.dst[7] = rm + im;
+  b.src[8] = rp + im; b.dst[8] = rm + ip;
+  return b;
+}
+
+// ------------------------------------------------------------------------------------------
+// (1) classification (one-time).  PAPER.md:21: fluid (solid) boundary node = has >= 1 solid
+// (fluid) neighbour in the D2Q9 stencil; periodic wrap.  Integer logic only => bit-exact.
+// cls == nullptr: count ghosts only (lbm_plan).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ mask, int nx, int ny,
+                                                  uint8_t* __restrict__ cls,
+                                                  uint8_t* __restrict__ links,
+                                                  int* __restrict__ block_count,
+                                                  unsigned long long* __restrict__ total) {
+  const long long n = (long long)nx * ny;
+  const long long k = (long long)blockIdx.x * 256 + threadIdx.x;
+  int is_ghost = 0;
+  if (k < n) {
+    const int i = (int)(k % nx), j = (int)(k / nx);
+    const Nbr b = make_nbr(i, j, nx, ny);
+    const int solid = mask[k] != 0;
+    unsigned lk = 0;
+    int other = 0;
+#pragma unroll
+    for (int q = 1; q < 9; q++) {
+      const int s = mask[b.src[q]] != 0;
+      lk |= (unsigned)s << (q - 1);
+      other |= (s != solid);
+    }
+    const uint8_t c = solid ? (other ? 2 : 3) : (other ? 1 : 0);
+    is_ghost = (c == 2);
+    if (cls) {
+      cls[k] = c;
+      links[k] = solid ? 0 : (uint8_t)lk;
+    }
+  }
+  const int cnt = __syncthreads_count(is_ghost);
+  if (threadIdx.x == 0) {
+    if (block_count) block_count[blockIdx.x] = cnt;
+    if (total && cnt) atomicAdd(total, (unsigned long long)cnt);
+  }
+}
+
+// exclusive scan of the per-block ghost counts (single block; one-time)
+__global__ void __launch_bounds__(1024) k_scan_blocks(const int* __restrict__ cnt, int nb,
+                                                      int* __restrict__ off, int* __restrict__ total) {
+  __shared__ int wsum[32];
+  __shared__ int carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int base = 0; base < nb; base += 1024) {
+    const int t = base + threadIdx.x;
+    const int v = t < nb ? cnt[t] : 0;
+    int x = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    if (w == 0) {
+      int s = wsum[lane];
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, s, d);
+        if (lane >= d) s += y;
+      }
+      wsum[lane] = s;  // inclusive over warps
+    }
+    __syncthreads();
+    const int wo = w ? wsum[w - 1] : 0;
+    if (t < nb) off[t] = carry + wo + x - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry += wo + x;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *total = carry;
+}
+
+// index-sorted compaction of ghost nodes
+__global__ void __launch_bounds__(256) k_compact_ghosts(const uint8_t* __restrict__ cls, long long n,
+                                                        const int* __restrict__ block_off,
+                                                        int* __restrict__ gidx) {
+  __shared__ int wcnt[8];
+  const long long k = (long long)blockIdx.x * 256 + threadIdx.x;
+  const int flag = (k < n) && (cls[k] == 2);
+  const unsigned bal = __ballot_sync(0xffffffffu, flag);
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) wcnt[w] = __popc(bal);
+  __syncthreads();
+  int wo = 0;
+  for (int v = 0; v < w; v++) wo += wcnt[v];
+  if (flag) gidx[block_off[blockIdx.x] + wo + __popc(bal & ((1u << lane) - 1u))] = (int)k;
+}
+
+// Per-ghost geometry (one-time): analytic unit normal of the owning disk / wall row (:100, :60),
+// depth, x_F = x_G + n_s (:66) and its bilinear stencil.  All in fp64 WITHOUT fma contraction so
+// that the list can be compared bit for bit.
+struct Disk { double cx, cy, r; };
+
+__device__ __forceinline__ double minimg_d(double d, double L) {
+  d = fmod(d, L);
+  if (d >= 0.5 * L) d = __dsub_rn(d, L);
+  if (d < -0.5 * L) d = __dadd_rn(d, L);
+  return d;
+}
+__device__ __forceinline__ int wrapi_d(int a, int n) {
+  a %= n;
+  return a < 0 ? a + n : a;
+}
+
+template <typename R>
+__global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __restrict__ gidx, int nx,
+                                                        int ny, int wall_rows,
+                                                        const Disk* __restrict__ disks, int n_disks,
+                                                        const uint8_t* __restrict__ cls,
+                                                        double* __restrict__ gnx, double* __restrict__ gny,
+                                                        double* __restrict__ gdepth,
+                                                        int* __restrict__ corner, double* __restrict__ wgt_d,
+                                                        R* __restrict__ wgt, uint8_t* __restrict__ csolid,
+                                                        int* __restrict__ err) {
+  const int g = blockIdx.x * 128 + threadIdx.x;
+  if (g >= ng) return;
+  const int k = gidx[g];
+  const int i = k % nx, j = k / nx;
+  double nxs = 0.0, nys = 0.0, depth = 0.0;
+  int found = 0;
+  if (wall_rows && (j == 0 || j == ny - 1)) {
+    nys = (j == 0) ? 1.0 : -1.0;
+    depth = 0.5;  // half-way wall (R17)
+    found = 1;
+  } else {
+    double best = 0.0;
+    for (int d = 0; d < n_disks; d++) {
+      const Disk dk = disks[d];
+      const double dx = minimg_d(__dsub_rn((double)i, dk.cx), (double)nx);
+      const double dy = minimg_d(__dsub_rn((double)j, dk.cy), (double)ny);
+      const double r2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+      if (r2 <= __dmul_rn(dk.r, dk.r)) {
+        const double dist = __dsqrt_rn(r2);
+        const double dep = __dsub_rn(dk.r, dist);
+        if (!found || dep < best) {
+          best = dep;
+          found = 1;
+          depth = dep;
+          if (dist > 0.0) { nxs = __ddiv_rn(dx, dist); nys = __ddiv_rn(dy, dist); }
+          else { nxs = 0.0; nys = 0.0; }
+        }
+      }
+    }
+  }
+  if (!found) atomicExch(err, 1);
+  gnx[g] = nxs; gny[g] = nys; gdepth[g] = depth;
+  const double xF = __dadd_rn((double)i, nxs), yF = __dadd_rn((double)j, nys);
+  const double fi = floor(xF), fj = floor(yF);
+  const double fx = __dsub_rn(xF, fi), fy = __dsub_rn(yF, fj);
+  const int i0 = wrapi_d((int)fi, nx), j0 = wrapi_d((int)fj, ny);
+  const int i1 = wrapi_d(i0 + 1, nx), j1 = wrapi_d(j0 + 1, ny);
+  const int c0 = j0 * nx + i0, c1 = j0 * nx + i1, c2 = j1 * nx + i0, c3 = j1 * nx + i1;
+  const double w0 = __dmul_rn(__dsub_rn(1.0, fx), __dsub_rn(1.0, fy));
+  const double w1 = __dmul_rn(fx, __dsub_rn(1.0, fy));
+  const double w2 = __dmul_rn(__dsub_rn(1.0, fx), fy);
+  const double w3 = __dmul_rn(fx, fy);
+  corner[4 * g + 0] = c0; corner[4 * g + 1] = c1; corner[4 * g + 2] = c2; corner[4 * g + 3] = c3;
+  wgt_d[4 * g + 0] = w0; wgt_d[4 * g + 1] = w1; wgt_d[4 * g + 2] = w2; wgt_d[4 * g + 3] = w3;
+  wgt[4 * g + 0] = (R)w0; wgt[4 * g + 1] = (R)w1; wgt[4 * g + 2] = (R)w2; wgt[4 * g + 3] = (R)w3;
+  csolid[g] = (uint8_t)((cls[c0] >= 2) | ((cls[c1] >= 2) << 1) | ((cls[c2] >= 2) << 2) | ((cls[c3] >= 2) << 3));
+}
+
+// ------------------------------------------------------------------------------------------
+// (2) ghost-node order-parameter update, Eq. 9 (:78-80): phi_F by bilinear interpolation at
+// x_F = x_G + n_s (:66); Jacobi (R13): fluid corners carry this time's phi (phi_cur), solid
+// corners the previous ghost values (phi_prev; bulk solid nodes are constant in both buffers).
+// ------------------------------------------------------------------------------------------
+template <typename R>
+__global__ void __launch_bounds__(128) k_ghost_update(const Consts<R> C, int ng,
+                                                      const int* __restrict__ gidx,
+                                                      const int4* __restrict__ corner,
+                                                      const R* __restrict__ wgt,
+                                                      const uint8_t* __restrict__ csolid,
+                                                      const R* __restrict__ phi_prev,
+                                                      R* __restrict__ phi_cur) {
+  const int g = blockIdx.x * 128 + threadIdx.x;
+  if (g >= ng) return;
+  const int4 c = corner[g];
+  const unsigned sb = csolid[g];
+  const R w0 = wgt[4 * g + 0], w1 = wgt[4 * g + 1], w2 = wgt[4 * g + 2], w3 = wgt[4 * g + 3];
+  const R p0 = (sb & 1u) ? phi_prev[c.x] : phi_cur[c.x];
+  const R p1 = (sb & 2u) ? phi_prev[c.y] : phi_cur[c.y];
+  const R p2 = (sb & 4u) ? phi_prev[c.z] : phi_cur[c.z];
+  const R p3 = (sb & 8u) ? phi_prev[c.w] : phi_cur[c.w];
+  const R phiF = ((w0 * p0 + w1 * p1) + w2 * p2) + w3 * p3;
+  phi_cur[gidx[g]] = ghost_rule<R>(C, phiF);
+}
+
+// ------------------------------------------------------------------------------------------
+// pulled (post-stream) population q of node k: propagation A16-A17 + half-way bounce-back (R12)
+// ------------------------------------------------------------------------------------------
+template <typename R>
+__device__ __forceinline__ void pull9(const R* __restrict__ pop, size_t n, int k, const Nbr& b,
+                                      unsigned lk, R (&v)[9]) {
+  v[0] = pop[k];
+  if (lk == 0) {
+#pragma unroll
+    for (int q = 1; q < 9; q++) v[q] = pop[q * n + b.src[q]];
+  } else {
+#pragma unroll
+    for (int q = 1; q < 9; q++)
+      v[q] = ((lk >> (q - 1)) & 1u) ? pop[opp(q) * n + k] : pop[q * n + b.src[q]];
+  }
+}
+
+template <typename R>
+__device__ __forceinline__ void load_phi9(const R* __restrict__ phi, const Nbr& b, R (&ph)[9]) {
+#pragma unroll
+  for (int q = 0; q < 9; q++) ph[q] = phi[b.dst[q]];
+}
+
+// ------------------------------------------------------------------------------------------
+// BASELINE schedule, kernel (3): fused pull-stream + collide, one thread per node.
+// Reads 9 pulled N, the 3x3 phi neighbourhood, 1 class byte; writes 9 N* and 9 B*.
+// ------------------------------------------------------------------------------------------
+template <typename R>
+__global__ void __launch_bounds__(256) k_collide_baseline(const Consts<R> C,
+                                                          const uint8_t* __restrict__ cls,
+                                                          const uint8_t* __restrict__ links,
+                                                          const R* __restrict__ Nsrc, R* __restrict__ Ndst,
+                                                          R* __restrict__ Bdst,
+                                                          const R* __restrict__ phi) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = (size_t)C.nx * C.ny;
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (c >= 2) return;
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  R nn[9], ph[9], ns[9], bs[9];
+  load_phi9<R>(phi, b, ph);
+  pull9<R>(Nsrc, n, k, b, lk, nn);
+  node_update<R, true>(C, nn, ph, ns, bs, nullptr);
+#pragma unroll
+  for (int q = 0; q < 9; q++) {
+    Ndst[q * n + k] = ns[q];
+    Bdst[q * n + k] = bs[q];
+  }
+}
+
+// BASELINE schedule: phi(x, t+1) = sum_i B_i(x, t+1) (A13, :311) from the pulled B*.
+template <typename R>
+__global__ void __launch_bounds__(256) k_phi_sum(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                 const uint8_t* __restrict__ links,
+                                                 const R* __restrict__ Bsrc, R* __restrict__ phi) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = (size_t)C.nx * C.ny;
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (c >= 2) return;
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  R v[9];
+  pull9<R>(Bsrc, n, k, b, lk, v);
+  R s = v[0];
+#pragma unroll
+  for (int q = 1; q < 9; q++) s += v[q];
+  phi[k] = s;
+}
+
+// ------------------------------------------------------------------------------------------
+// init (R14): N_i(x, 0) = N_i^eq(p = 0, u0(x)) (Eq. A4), B_i = phi0 N_i; stored "un-streamed" so
+// that the pull of the first step returns exactly these values: slot (q, y) holds N_q(y + c_q, 0)
+// if y + c_q is fluid, else N_opp(q)(y, 0) (the value the bounce-back link will hand back).
+// ------------------------------------------------------------------------------------------
+template <typename R>
+__device__ __forceinline__ R neq_dev_p0(int q, R ux, R uy) {
+  // deviation of Eq. A4 at p = 0
+  const int cx[9] = {0, 1, 0, -1, 0, 1, -1, -1, 1}, cy[9] = {0, 0, 1, 0, -1, 1, 1, -1, -1};
+  const R u2 = ux * ux + uy * uy;
+  if (q == 0) return R(-2.0 / 3.0) * u2;
+  const R w = q < 5 ? R(1.0 / 9.0) : R(1.0 / 36.0);
+  const R cu = cx[q] * ux + cy[q] * uy;
+  return w * (R(3.0) * cu + R(4.5) * cu * cu - R(1.5) * u2);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                              const uint8_t* __restrict__ links,
+                                              const double* __restrict__ phi0,
+                                              const double* __restrict__ u0, R* __restrict__ Npop,
+                                              R* __restrict__ Bpop, R* __restrict__ phiA,
+                                              R* __restrict__ phiB) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = (size_t)C.nx * C.ny;
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (c >= 2) {
+    phiA[k] = C.phi_solid;
+    phiB[k] = C.phi_solid;
+#pragma unroll
+    for (int q = 0; q < 9; q++) {
+      Npop[q * n + k] = R(0);
+      if (Bpop) Bpop[q * n + k] = R(0);
+    }
+    return;
+  }
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const R chi[9] = {C.chi0, C.chi1, C.chi1, C.chi1, C.chi1, C.chi5, C.chi5, C.chi5, C.chi5};
+  R s = R(0);
+#pragma unroll
+  for (int q = 0; q < 9; q++) {
+    // is y + c_q solid?  y + c_q = y - c_opp(q): link bit of opp(q)
+    const int oq = opp(q);
+    const bool blocked = q > 0 && ((lk >> (oq - 1)) & 1u);
+    const int src = blocked ? k : b.dst[q];
+    const int qq = blocked ? oq : q;
+    const R ux = u0 ? (R)u0[src] : R(0), uy = u0 ? (R)u0[n + src] : R(0);
+    const R dev = neq_dev_p0<R>(qq, ux, uy);
+    Npop[q * n + k] = dev;
+    if (Bpop) Bpop[q * n + k] = (R)phi0[src] * (chi[qq] + dev);
+    // phi(x, 0) = sum_i B_i(x, 0) = sum_i phi0(x) N_i^eq(u0(x)) in the oracle's order (A13)
+    const R uxk = u0 ? (R)u0[k] : R(0), uyk = u0 ? (R)u0[n + k] : R(0);
+    s += (R)phi0[k] * (chi[q] + neq_dev_p0<R>(q, uxk, uyk));
+  }
+  phiA[k] = s;
+  phiB[k] = s;
+}
+
+// ------------------------------------------------------------------------------------------
+// lbm_get: macroscopic fields at the current time into double staging planes
+// ------------------------------------------------------------------------------------------
+template <typename R>
+__global__ void __launch_bounds__(256) k_moments(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                 const uint8_t* __restrict__ links,
+                                                 const R* __restrict__ Nsrc, const R* __restrict__ phi,
+                                                 double* __restrict__ o_rho, double* __restrict__ o_phi,
+                                                 double* __restrict__ o_ux, double* __restrict__ o_uy,
+                                                 double* __restrict__ o_p) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = (size_t)C.nx * C.ny;
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (o_phi) o_phi[k] = (double)phi[k];
+  if (c >= 2) {
+    if (o_rho) o_rho[k] = 0.0;
+    if (o_ux) o_ux[k] = 0.0;
+    if (o_uy) o_uy[k] = 0.0;
+    if (o_p) o_p[k] = 0.0;
+    return;
+  }
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  R nn[9], ph[9], ns[9], bs[9];
+  NodeOut<R> o;
+  load_phi9<R>(phi, b, ph);
+  pull9<R>(Nsrc, n, k, b, lk, nn);
+  node_update<R, false>(C, nn, ph, ns, bs, &o);
+  if (o_rho) o_rho[k] = (double)o.rho;
+  if (o_ux) o_ux[k] = (double)o.ux;
+  if (o_uy) o_uy[k] = (double)o.uy;
+  if (o_p) o_p[k] = (double)o.p;
+}
+
+// post-stream population plane q (full N_q = chi_q + deviation, or B_q) into a double plane
+template <typename R>
+__global__ void __launch_bounds__(256) k_gather_plane(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                      const uint8_t* __restrict__ links,
+                                                      const R* __restrict__ pop, int q, double add,
+                                                      double* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = (size_t)C.nx * C.ny;
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (c >= 2) { out[k] = 0.0; return; }
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  R v;
+  if (q == 0) v = pop[k];
+  else v = ((lk >> (q - 1)) & 1u) ? pop[opp(q) * n + k] : pop[q * n + b.src[q]];
+  out[k] = (double)v + add;
+}
+
+// same at selected nodes: out[q*m + t]
+template <typename R>
+__global__ void __launch_bounds__(128) k_gather_samples(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                        const uint8_t* __restrict__ links,
+                                                        const R* __restrict__ pop, int add_chi,
+                                                        long long m, const long long* __restrict__ idx,
+                                                        double* __restrict__ out) {
+  const long long t = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (t >= m) return;
+  const size_t n = (size_t)C.nx * C.ny;
+  const int k = (int)idx[t];
+  const uint8_t c = cls[k];
+  const Nbr b = make_nbr(k % C.nx, k / C.nx, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const double chi[9] = {(double)C.chi0, (double)C.chi1, (double)C.chi1, (double)C.chi1, (double)C.chi1,
+                         (double)C.chi5, (double)C.chi5, (double)C.chi5, (double)C.chi5};
+  for (int q = 0; q < 9; q++) {
+    double v = 0.0;
+    if (c < 2) {
+      R x;
+      if (q == 0) x = pop[k];
+      else x = ((lk >> (q - 1)) & 1u) ? pop[opp(q) * n + k] : pop[q * n + b.src[q]];
+      v = (double)x + (add_chi ? chi[q] : 0.0);
+    }
+    out[q * m + t] = v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// (a8) diagnostics: warp-shuffle + fixed-tree block reduction into per-block partials, then a
+// single-block fixed-order pass.  Deterministic for a given grid.
+// partial layout: [6][nblocks]: sum phi, sum (1-phi), KE, max|u|^2, min phi, max phi; + count, nan
+// ------------------------------------------------------------------------------------------
+struct DiagVec { double s_phi, s_omp, ke, umax2, pmin, pmax, cnt, bad; };
+
+__device__ __forceinline__ DiagVec diag_combine(const DiagVec& a, const DiagVec& b) {
+  DiagVec r;
+  r.s_phi = a.s_phi + b.s_phi; r.s_omp = a.s_omp + b.s_omp; r.ke = a.ke + b.ke;
+  r.umax2 = fmax(a.umax2, b.umax2); r.pmin = fmin(a.pmin, b.pmin); r.pmax = fmax(a.pmax, b.pmax);
+  r.cnt = a.cnt + b.cnt; r.bad = fmax(a.bad, b.bad);
+  return r;
+}
+__device__ __forceinline__ DiagVec diag_shfl_down(const DiagVec& a, int d) {
+  DiagVec r;
+  r.s_phi = __shfl_down_sync(0xffffffffu, a.s_phi, d); r.s_omp = __shfl_down_sync(0xffffffffu, a.s_omp, d);
+  r.ke = __shfl_down_sync(0xffffffffu, a.ke, d); r.umax2 = __shfl_down_sync(0xffffffffu, a.umax2, d);
+  r.pmin = __shfl_down_sync(0xffffffffu, a.pmin, d); r.pmax = __shfl_down_sync(0xffffffffu, a.pmax, d);
+  r.cnt = __shfl_down_sync(0xffffffffu, a.cnt, d); r.bad = __shfl_down_sync(0xffffffffu, a.bad, d);
+  return r;
+}
+__device__ __forceinline__ DiagVec diag_identity() {
+  DiagVec r;
+  r.s_phi = 0; r.s_omp = 0; r.ke = 0; r.umax2 = 0; r.cnt = 0; r.bad = 0;
+  r.pmin = __longlong_as_double(0x7ff0000000000000LL); r.pmax = -r.pmin;
+  return r;
+}
+__device__ __forceinline__ DiagVec diag_block_reduce(DiagVec v, DiagVec* sh) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v = diag_combine(v, diag_shfl_down(v, d));
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  if (lane == 0) sh[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    v = lane < nw ? sh[lane] : diag_identity();
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v = diag_combine(v, diag_shfl_down(v, d));
+  }
+  return v;  // valid in thread 0
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) k_diag_partial(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                      const uint8_t* __restrict__ links,
+                                                      const R* __restrict__ Nsrc, const R* __restrict__ phi,
+                                                      DiagVec* __restrict__ partial) {
+  __shared__ DiagVec sh[32];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  DiagVec v = diag_identity();
+  if (i < C.nx) {
+    const size_t n = (size_t)C.nx * C.ny;
+    const int k = j * C.nx + i;
+    const uint8_t c = cls[k];
+    if (c < 2) {
+      const Nbr b = make_nbr(i, j, C.nx, C.ny);
+      const unsigned lk = (c == 1) ? links[k] : 0u;
+      R nn[9], ph[9], ns[9], bs[9];
+      NodeOut<R> o;
+      load_phi9<R>(phi, b, ph);
+      pull9<R>(Nsrc, n, k, b, lk, nn);
+      node_update<R, false>(C, nn, ph, ns, bs, &o);
+      const double f = (double)ph[0], ux = (double)o.ux, uy = (double)o.uy;
+      const double u2 = ux * ux + uy * uy;
+      v.s_phi = f; v.s_omp = 1.0 - f; v.ke = 0.5 * (double)o.rho * u2; v.umax2 = u2;
+      v.pmin = f; v.pmax = f; v.cnt = 1.0;
+      v.bad = (f != f || u2 != u2) ? 1.0 : 0.0;
+      if (v.bad != 0.0) { v.umax2 = 0.0; v.pmin = diag_identity().pmin; v.pmax = -v.pmin; }
+    }
+  }
+  v = diag_block_reduce(v, sh);
+  if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = v;
+}
+
+__global__ void __launch_bounds__(1024) k_diag_final(const DiagVec* __restrict__ partial, long long m,
+                                                     double* __restrict__ out) {
+  __shared__ DiagVec sh[32];
+  DiagVec v = diag_identity();
+  for (long long t = threadIdx.x; t < m; t += 1024) v = diag_combine(v, partial[t]);
+  v = diag_block_reduce(v, sh);
+  if (threadIdx.x == 0) {
+    out[0] = v.s_phi; out[1] = v.s_omp; out[2] = v.ke; out[3] = sqrt(v.umax2);
+    out[4] = v.pmin; out[5] = v.pmax; out[6] = v.cnt; out[7] = v.bad;
+  }
+}
+
+// test hook: independent nodes
+template <typename R>
+__global__ void __launch_bounds__(128) k_node_batch(const Consts<R> C, long long count,
+                                                    const double* __restrict__ Nin,
+                                                    const double* __restrict__ phin,
+                                                    double* __restrict__ Ns, double* __restrict__ Bs,
+                                                    double* __restrict__ fields) {
+  const long long t = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (t >= count) return;
+  const R chi[9] = {C.chi0, C.chi1, C.chi1, C.chi1, C.chi1, C.chi5, C.chi5, C.chi5, C.chi5};
+  const double chid[9] = {(double)C.chi0, (double)C.chi1, (double)C.chi1, (double)C.chi1, (double)C.chi1,
+                          (double)C.chi5, (double)C.chi5, (double)C.chi5, (double)C.chi5};
+  R nn[9], ph[9], ns[9], bs[9];
+  NodeOut<R> o;
+  for (int q = 0; q < 9; q++) {
+    nn[q] = (R)(Nin[9 * t + q] - chid[q]);   // deviation taken in double, then rounded
+    ph[q] = (R)phin[9 * t + q];
+  }
+  (void)chi;
+  node_update<R, true>(C, nn, ph, ns, bs, &o);
+  for (int q = 0; q < 9; q++) {
+    if (Ns) Ns[9 * t + q] = (double)ns[q] + chid[q];
+    if (Bs) Bs[9 * t + q] = (double)bs[q];
+  }
+  if (fields) {
+    double* f = fields + 8 * t;
+    f[0] = o.rho; f[1] = o.tau; f[2] = o.ux; f[3] = o.uy; f[4] = o.p; f[5] = o.Fx; f[6] = o.Fy; f[7] = o.gnorm;
+  }
+}
+
+}  // namespace lbm

@@ -1,0 +1,61 @@
+"""Host-side checks that need no GPU: the C-ABI library builds for sm_100a, loads, and exports every
+symbol include/lbm.h declares; parameter validation happens before any CUDA call."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+from paper_2605_30878_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    txt = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(lbm_[a-z_A-Z0-9]+)\s*\(", txt)))
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    binding.build_library()
+    lib = binding.load_library()
+    names = _declared()
+    assert len(names) >= 14
+    for name in names:
+        assert hasattr(lib, name), name
+    assert set(names) == set(binding.EXPORTS)
+    assert b"sm_100a" in lib.lbm_version()
+
+
+def test_params_struct_layout_matches_header():
+    # 6 int32 then 10 doubles, no padding surprises
+    assert C.sizeof(binding._Params) == 6 * 4 + 10 * 8
+    assert binding._Params.rho_l.offset == 24
+
+
+def test_validation_precedes_cuda():
+    lib = binding.load_library()
+    mask = np.zeros(64, np.uint8)
+    ng, ws = C.c_int64(), C.c_size_t()
+    bad = [dict(W=3.0), dict(nu_l=0.0), dict(precision=16), dict(nx=2), dict(theta_deg=200.0),
+           dict(mobility=0.5), dict(rho_g=-1.0), dict(ghost_rule=3), dict(schedule=9), dict(wall_rows=1)]
+    for kw in bad:
+        d = dict(nx=8, ny=8); d.update(kw)
+        ps = binding.LBMParams(**d).c_struct()
+        rc = lib.lbm_plan(C.byref(ps), mask.ctypes.data, C.byref(ng), C.byref(ws))
+        assert rc == -1, kw
+        assert len(lib.lbm_last_error(None)) > 0
+    h = C.c_void_p()
+    ps = binding.LBMParams(nx=8, ny=8).c_struct()
+    assert lib.lbm_create(C.byref(h), C.byref(ps), mask.ctypes.data, None, 0, None, 0, None) == -1
+    assert lib.lbm_step(None, 1) == -1 and lib.lbm_init(None, None, None) == -1
+
+
+def test_no_cpu_fallback_without_device():
+    import pytest
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(binding.LBMError):
+        binding.LBM(binding.LBMParams(nx=8, ny=8), np.zeros((8, 8), np.uint8))

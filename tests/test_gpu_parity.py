@@ -1,0 +1,295 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances: classification and ghost
+geometry bit-exact; fp64 fields and populations <= 1e-10 absolute after 1,000 steps (north_star);
+fp32 <= 2e-4 relative to field scale against the fp64 oracle."""
+import math
+
+import numpy as np
+import pytest
+
+import _measure as ms
+from _parity import ArrayWorkload, field_errors, make_pair, pop_errors
+from paper_2605_30878_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+BASELINE, FUSED = 1, 2
+SCHEDULES = [pytest.param(BASELINE, id="baseline"), pytest.param(FUSED, id="fused")]
+
+
+# ---- local update of single nodes ---------------------------------------------------------------
+def _random_nodes(count, seed):
+    from oracle import ref
+    rng = np.random.default_rng(seed)
+    chi = ref.chi(14 / 15)
+    N = chi[None, :] + rng.normal(0, 1e-3, (count, 9))
+    base = rng.uniform(0, 1, (count, 1))
+    nb = np.clip(base + rng.normal(0, 0.05, (count, 9)), -0.01, 1.01)
+    nb[:4] = [[0] * 9, [1] * 9, [0.5] * 9, [0.3] * 9]           # uniform phi: zero gradient (R16)
+    return N, nb
+
+
+@pytest.mark.parametrize("prm", [dict(rho_l=1.0, nu_l=1 / 6, nu_g=1 / 6), dict(rho_l=1000.0, nu_l=0.01, nu_g=0.1),
+                                 dict(rho_l=100.0, nu_l=0.01, nu_g=0.1, gx=1e-5, gy=-2e-5, W=5.0, sigma=0.02)])
+def test_node_update_fp64(prm):
+    from oracle import ref
+    from paper_2605_30878_b200 import binding
+    N, nb = _random_nodes(300, 3)
+    Ns, Bs, F = binding.node_update_batch(binding.LBMParams(nx=8, ny=8, precision=64, **prm), N, nb)
+    rp = ref.RefParams(nx=8, ny=8, **prm)
+    worst = 0.0
+    for k in range(N.shape[0]):
+        oN, oB, f = ref.node_update(rp, N[k], nb[k])
+        worst = max(worst, np.abs(Ns[k] - oN).max(), np.abs(Bs[k] - oB).max())
+        assert abs(F["ux"][k] - f.ux) < 1e-14 and abs(F["uy"][k] - f.uy) < 1e-14
+        assert abs(F["p"][k] - f.p) < 1e-14 and abs(F["rho"][k] - f.rho) < 1e-11
+        assert abs(F["tau"][k] - f.tau) < 1e-13
+        assert abs(F["Fx"][k] - f.Fx) < 1e-13 * max(1.0, prm["rho_l"])
+    assert worst < 5e-15, worst
+
+
+def test_node_update_fp32():
+    from oracle import ref
+    from paper_2605_30878_b200 import binding
+    prm = dict(rho_l=1000.0, nu_l=0.01, nu_g=0.1)
+    N, nb = _random_nodes(200, 4)
+    Ns, Bs, F = binding.node_update_batch(binding.LBMParams(nx=8, ny=8, precision=32, **prm), N, nb)
+    rp = ref.RefParams(nx=8, ny=8, **prm)
+    for k in range(N.shape[0]):
+        oN, oB, f = ref.node_update(rp, N[k], nb[k])
+        assert np.abs(Ns[k] - oN).max() < 2e-6      # deviations ~1e-3 carried in fp32, phi in fp32
+        assert np.abs(Bs[k] - oB).max() < 2e-6
+        assert abs(F["p"][k] - f.p) < 2e-6
+
+
+# ---- classification and ghost geometry: bit-exact ------------------------------------------------
+def _mask_cases():
+    rng = np.random.default_rng(11)
+    cases = {}
+    cases["empty"] = np.zeros((8, 9), np.uint8)
+    cases["full"] = np.ones((8, 9), np.uint8)
+    m = np.zeros((9, 8), np.uint8); m[4, 3] = 1
+    cases["single_node"] = m
+    m = np.ones((9, 8), np.uint8); m[0, 0] = 0
+    cases["single_fluid_corner"] = m
+    yy, xx = np.mgrid[0:10, 0:12]
+    cases["checkerboard"] = ((xx + yy) % 2).astype(np.uint8)
+    cases["seam_disk"] = wl.rasterize_disks(32, 24, [[0.3, 23.6, 6.0]])
+    for k in range(4):
+        cases[f"random{k}"] = (rng.uniform(size=(8 + k, 13 - k)) < 0.3 + 0.1 * k).astype(np.uint8)
+    cases["random_big"] = (rng.uniform(size=(37, 300)) < 0.3).astype(np.uint8)   # several 256-blocks, ragged
+    return cases
+
+
+def _assert_same_classification(a, b):
+    assert np.array_equal(a["cls"], b["cls"])
+    assert a["n_ghost"] == b["n_ghost"]
+    assert np.array_equal(a["idx"], b["idx"])
+    assert np.array_equal(a["corner"], b["corner"])
+    for k in ("nx", "ny", "depth", "wgt"):
+        assert np.array_equal(a[k], b[k]), k            # fp64 geometry without contraction: bit-exact
+
+
+@pytest.mark.parametrize("name", list(_mask_cases().keys()))
+def test_classification_masks_bit_exact(name):
+    mask = _mask_cases()[name]
+    ny, nx = mask.shape
+    w = ArrayWorkload(mask, np.zeros((ny, nx)), disks=[[nx / 2, ny / 2, 10 * (nx + ny)]])
+    g, o = make_pair(w)
+    _assert_same_classification(g.get_classification(), o.get_classification())
+
+
+@pytest.mark.parametrize("make", [lambda: wl.config1(seed=1), lambda: wl.config2(seed=3, theta_deg=120.0),
+                                  lambda: wl.config4(seed=2, nx=512, ny=128), lambda: wl.config5(seed=1, n=512)],
+                         ids=["config1", "config2", "config4_small", "config5_512"])
+def test_classification_configs_bit_exact(make):
+    w = make()
+    g, o = make_pair(w, precision=32)          # geometry is fp64 in both precisions
+    _assert_same_classification(g.get_classification(), o.get_classification())
+
+
+# ---- one call of each kernel ---------------------------------------------------------------------
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_init_and_first_ghost_update(schedule):
+    w = wl.config1(seed=2)
+    g, o = make_pair(w, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    fluid = w.mask == 0
+    eN, eB = pop_errors(g, o, fluid)
+    assert eN < 1e-16 and eB < 1e-16
+    err, _ = field_errors(g, o)
+    assert err["phi"] < 1e-15, err            # includes the ghost values of Eq. 9
+    assert max(err["ux"], err["uy"], err["p"]) < 1e-15 and err["rho"] < 1e-13
+
+
+def test_init_with_velocity():
+    w = wl.config2(seed=1, theta_deg=60.0, n=64)
+    rng = np.random.default_rng(0)
+    u0 = rng.normal(0, 1e-3, (2, w.ny, w.nx))
+    g, o = make_pair(w, schedule=BASELINE)
+    g.init(w.phi0, u0); o.init(w.phi0, u0)
+    eN, eB = pop_errors(g, o, w.mask == 0)
+    assert eN < 1e-16 and eB < 1e-16
+
+
+@pytest.mark.parametrize("schedule", SCHEDULES)
+@pytest.mark.parametrize("steps", [1, 2, 7])
+def test_few_steps_config1(schedule, steps):
+    w = wl.config1(seed=0)
+    g, o = make_pair(w, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    g.keep_B(True)
+    g.step(steps); o.step(steps)
+    eN, eB = pop_errors(g, o, w.mask == 0)
+    err, _ = field_errors(g, o)
+    assert eN < 1e-14 and eB < 1e-14, (eN, eB)
+    assert max(err.values()) < 1e-14, err
+
+
+# ---- edge cases: ragged sizes across several tiles, random masks, walls, tiny grids ---------------
+def _random_case(ny, nx, seed, frac=0.25, **prm):
+    rng = np.random.default_rng(seed)
+    mask = (rng.uniform(size=(ny, nx)) < frac).astype(np.uint8)
+    phi0 = rng.uniform(0, 1, (ny, nx))
+    # smooth phi0 a little so that gradients are moderate
+    for _ in range(2):
+        phi0 = 0.25 * (np.roll(phi0, 1, 0) + np.roll(phi0, -1, 0) + np.roll(phi0, 1, 1) + np.roll(phi0, -1, 1))
+    return ArrayWorkload(mask, phi0, disks=[[nx / 2 + 0.3, ny / 2 + 0.2, 10 * (nx + ny)]], **prm)
+
+
+@pytest.mark.parametrize("schedule", SCHEDULES)
+@pytest.mark.parametrize("shape,frac", [((3, 3), 0.0), ((5, 4), 0.3), ((45, 70), 0.25), ((70, 300), 0.3),
+                                        ((19, 127), 0.5), ((9, 126), 0.1), ((130, 253), 0.2)])
+def test_random_masks_ragged(schedule, shape, frac):
+    w = _random_case(shape[0], shape[1], seed=shape[0] * 1000 + shape[1], frac=frac, rho_l=20.0, nu_l=0.05)
+    g, o = make_pair(w, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    g.keep_B(True)
+    g.step(5); o.step(5)
+    fluid = w.mask == 0
+    if fluid.any():
+        eN, eB = pop_errors(g, o, fluid)
+        assert eN < 1e-13 and eB < 1e-13, (eN, eB)
+    err, _ = field_errors(g, o)
+    assert max(err.values()) < 1e-12, err
+
+
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_all_solid_and_all_fluid(schedule):
+    for mask in (np.ones((6, 7), np.uint8), np.zeros((6, 7), np.uint8)):
+        w = ArrayWorkload(mask, np.full((6, 7), 0.4), disks=[[3.3, 3.1, 100.0]])
+        g, o = make_pair(w, schedule=schedule)
+        g.init(w.phi0); o.init(w.phi0)
+        g.step(3); o.step(3)
+        err, _ = field_errors(g, o)
+        assert max(err.values()) < 1e-14, err
+
+
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_channel_with_walls_posts_body_force(schedule):
+    w = wl.config4(seed=2, nx=256, ny=64)
+    g, o = make_pair(w, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    g.keep_B(True)
+    g.step(40); o.step(40)
+    eN, eB = pop_errors(g, o, w.mask == 0)
+    err, _ = field_errors(g, o)
+    assert eN < 1e-12 and eB < 1e-12 and max(err.values()) < 1e-11, (eN, eB, err)
+    dg, do = g.diag(), o.diag()
+    assert dg["n_fluid"] == do["n_fluid"] and dg["nan"] == 0
+    assert abs(dg["sum_phi"] - do["sum_phi"]) < 1e-9 and abs(dg["umax"] - do["umax"]) < 1e-13
+    assert abs(dg["ke"] - do["ke"]) < 1e-12 * max(1.0, do["ke"])
+
+
+def test_fakhari_rule_variant():
+    w = wl.config2(seed=1, theta_deg=150.0, n=64)
+    for th in (150.0, 90.0):
+        g, o = make_pair(w, schedule=FUSED, ghost_rule=1, theta_deg=th)
+        g.init(w.phi0); o.init(w.phi0)
+        g.step(10); o.step(10)
+        err, _ = field_errors(g, o)
+        assert max(err.values()) < 1e-13, (th, err)
+
+
+# ---- the north-star parity run: config 1, 1,000 steps, fp64 <= 1e-10 ------------------------------
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_config1_1000_steps_fp64(schedule):
+    w = wl.config1(seed=0)
+    g, o = make_pair(w, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    g.keep_B(True)
+    g.step(1000); o.step(1000)
+    eN, eB = pop_errors(g, o, w.mask == 0)
+    err, scale = field_errors(g, o)
+    print("config1 1000 steps", schedule, eN, eB, err)
+    assert eN <= 1e-10 and eB <= 1e-10
+    assert max(err.values()) <= 1e-10, err
+    # mass of each phase conserved on the device too
+    m0 = float(w.phi0[w.mask == 0].sum())
+    assert abs(g.diag()["sum_phi"] - m0) < 1e-10 * m0
+
+
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_config1_1000_steps_fp32(schedule):
+    w = wl.config1(seed=0)
+    g, o = make_pair(w, precision=32, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    g.step(1000); o.step(1000)
+    err, scale = field_errors(g, o)
+    uscale = max(scale["ux"], scale["uy"], w.sigma / (w.rho_l * w.nu_l))        # R22
+    print("config1 fp32", schedule, err, scale)
+    assert err["phi"] <= 2e-4 and err["rho"] <= 2e-4 * scale["rho"]
+    assert max(err["ux"], err["uy"]) <= 2e-4 * uscale
+    Ng, _ = g.get_populations(want_B=False)
+    No, _ = o.get_populations()
+    assert np.abs(Ng - No)[:, w.mask == 0].max() <= 2e-4
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_config2_high_density_ratio_and_contact_angle(precision):
+    """Density ratio 10, W = 5, theta = 120: fields after 2,000 steps and the measured contact
+    angle (circle fit, §III.B) agree with the oracle within 0.5 deg (north_star)."""
+    w = wl.config2(seed=0, theta_deg=120.0, n=128)
+    g, o = make_pair(w, precision=precision)
+    g.init(w.phi0); o.init(w.phi0)
+    g.step(2000); o.step(2000)
+    a, b = g.get(), o.get()
+    tg = ms.contact_angle_on_cylinder(a["phi"], w.mask, w.disks[0], w.W)[0]
+    to = ms.contact_angle_on_cylinder(b["phi"], w.mask, w.disks[0], w.W)[0]
+    err, scale = field_errors(g, o)
+    print("config2", precision, err, tg, to)
+    assert abs(tg - to) <= 0.5
+    if precision == 64:
+        assert max(err.values()) <= 1e-10, err
+    else:
+        uscale = max(scale["ux"], scale["uy"], w.sigma / (w.rho_l * w.nu_l))
+        assert err["phi"] <= 2e-4 and max(err["ux"], err["uy"]) <= 2e-4 * uscale
+
+
+def test_config3_density_ratio_1000_short():
+    w = wl.config3(seed=0, n=256)
+    for precision, tol in ((64, 1e-10), (32, 2e-4)):
+        g, o = make_pair(w, precision=precision)
+        g.init(w.phi0); o.init(w.phi0)
+        g.step(300); o.step(300)
+        err, scale = field_errors(g, o)
+        uscale = max(scale["ux"], scale["uy"], w.sigma / (w.rho_l * w.nu_l))
+        print("config3", precision, err, scale)
+        assert err["phi"] <= tol
+        assert max(err["ux"], err["uy"]) <= (tol if precision == 64 else tol * uscale)
+        assert err["rho"] <= tol * (1.0 if precision == 64 else scale["rho"])
+
+
+def test_schedules_agree_and_get_is_idempotent():
+    w = wl.config5(seed=3, n=256)
+    a, _ = make_pair(w, schedule=BASELINE)
+    b, _ = make_pair(w, schedule=FUSED)
+    a.init(w.phi0); b.init(w.phi0)
+    a.step(25); b.step(10); b.get(); b.step(15)        # lbm_get must not disturb the state
+    fa, fb = a.get(), b.get()
+    for k in fa:
+        assert np.abs(fa[k] - fb[k]).max() < 1e-13, k
+    with pytest.raises(Exception):
+        b.get_populations(want_B=True)                 # B is not stored unless keep_B was set
+    lc = b.launch_counts()
+    assert lc["collide"] == 25 and lc["phi_sum"] == 0 and lc["ghost"] == 26
