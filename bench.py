@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the hot path (one LBM time step = collide+stream(+phi) and ghost update)
+on BASELINE.json's config 5 (porous medium, density ratio 1000, theta = 110 deg) at 8192^2.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--n 8192] [--precision 64|32|both] [--schedule auto|baseline|fused]
+
+Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement"):
+  value        MLUPS (Eq. 14: all grid nodes x steps / time / 1e6), device-resident state,
+               timed with CUDA events on the stream the kernels run on, max over ranks
+  e2e          the same metric through the C ABI with HOST buffers: lbm_init(phi0) -> lbm_step(K) ->
+               lbm_get(rho, phi, ux, uy, p), host<->device copies inside the timed region
+  roofline     dominant kernel (collide+stream): algorithmic bytes per launch / its CUDA-event duration
+               against the measured HBM copy bandwidth (MEASURED_PEAKS.json)
+  cpu_baseline the CPU oracle timed on this box's host cores on a bounded sample (N = 1, rank 0 only)
+Multi-GPU: the path does not shard in this build ("replicas only"): N independent replicas.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2605_30878_b200 import workloads as wl  # noqa: E402
+
+METRIC = "MLUPS (Eq. 14: grid nodes x steps / s / 1e6), D2Q9 color-gradient step with ghost-node wetting"
+FALLBACK_HBM_GBS = 6650.0
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, f"/tmp/lbm_clocks_{os.getpid()}_{index}.csv"
+
+    def start(self):
+        try:
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=self.fh,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.fh.close()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        try:
+            for line in open(self.path):
+                parts = [x.strip() for x in line.split(",")]
+                if len(parts) < 6:
+                    continue
+                try:
+                    sm.append(float(parts[0])); mx.append(float(parts[1]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, parts[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.remove(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def cpu_oracle_rate(steps: int, warmup: int, budget_s: float = 25.0):
+    """The oracle as it stands (single thread, fp64) on a bounded sample of config 5."""
+    from oracle import ref
+    # probe at 256^2 to size the sample
+    w = wl.config5(seed=0, n=256)
+    o = ref.RefLBM(ref.RefParams(**w.param_dict()), w.mask, w.disks)
+    o.init(w.phi0)
+    t = time.perf_counter(); o.step(2); rate = 2 * 256 * 256 / (time.perf_counter() - t)
+    n = 256
+    for cand in (512, 1024, 2048):
+        if (steps + warmup) * cand * cand / rate <= budget_s:
+            n = cand
+    while steps > 1 and (steps + warmup) * n * n / rate > budget_s:
+        steps = max(1, steps // 2)
+    w = wl.config5(seed=0, n=n)
+    o = ref.RefLBM(ref.RefParams(**w.param_dict()), w.mask, w.disks)
+    o.init(w.phi0)
+    o.step(warmup)
+    t = time.perf_counter(); o.step(steps); dt = time.perf_counter() - t
+    return dict(value=n * n * steps / dt / 1e6, unit="MLUPS", cores=1, kind="oracle",
+                sample=f"config5 recipe at {n}x{n} (same porosity, disk radii, blob fill), {steps} steps after "
+                       f"{warmup} warm-up, oracle/lbmref.c single thread fp64",
+                mflups=w.meta["n_fluid"] * steps / dt / 1e6, ms_per_step=dt / steps * 1e3, steps=steps, n=n)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, args.steps)
+    cb = cpu_oracle_rate(steps, max(0, min(args.warmup, 3)), budget_s=120.0)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": "MLUPS", "n_gpus": args.gpus,
+            "steps": cb["steps"], "warmup": min(args.warmup, 3), "ms_per_step": cb["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config5 porous medium, CPU-oracle sample {cb['n']}x{cb['n']}",
+                       "full_workload": f"config5 porous medium {args.n}x{args.n}"},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": cb["value"], "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def bench_precision(args, w, precision, schedule, device_index, dist):
+    import torch
+    from paper_2605_30878_b200 import binding
+
+    n = w.nx * w.ny
+    n_fluid = int(w.meta["n_fluid"])
+    rs = 8 if precision == 64 else 4
+    prm = binding.LBMParams(precision=precision, schedule=schedule, **w.param_dict())
+    t0 = time.perf_counter()
+    sim = binding.LBM(prm, w.mask, w.disks)
+    t_create = time.perf_counter() - t0
+
+    # pinned host buffers for the e2e leg (and for init)
+    phi0_h = torch.empty(n, dtype=torch.float64).pin_memory()
+    phi0_h.numpy()[:] = w.phi0.reshape(-1)
+    out_h = {k: torch.empty(n, dtype=torch.float64).pin_memory() for k in ("rho", "phi", "ux", "uy", "p")}
+    out_np = {k: v.numpy().reshape(w.ny, w.nx) for k, v in out_h.items()}
+
+    sim.init(phi0_h.numpy())
+    sim.step(args.warmup)
+    sim.sync()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps between two events on the launching stream ----
+    sampler = ClockSampler(device_index)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.launch_counts(reset=True)
+    barrier()
+    sampler.start()
+    e0.record()
+    sim.step(args.steps)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = sim.launch_counts()
+    n_launch = launches["collide"] + launches["phi_sum"] + launches["ghost"]
+
+    # ---- per-kernel split (CUDA events around every launch) ----
+    ks = min(args.steps, 50)
+    split = sim.step_timed(ks)
+    t_collide = split["collide"] / ks * 1e-3          # s per launch of the dominant kernel
+
+    # ---- e2e through the C ABI with host buffers ----
+    barrier()
+    t0 = time.perf_counter()
+    sim.init(phi0_h.numpy())
+    sim.step(args.steps)
+    sim.get(out=out_np)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    dg = sim.diag()
+
+    if dist is not None:
+        tt = torch.tensor([ms, t_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms, t_e2e = float(tt[0]), float(tt[1])
+
+    fused = schedule != binding.SCHEDULE_BASELINE
+    values = 20 if fused else 38
+    bytes_layout = n_fluid * values * rs + n          # + 1 class byte per node
+    bytes_canon = n_fluid * (36 * rs + 1)
+    peak, peak_src = measured_peak()
+    ach = bytes_layout / t_collide / 1e9
+    res = dict(
+        ms=ms, t_e2e=t_e2e, mlups=n * args.steps / (ms * 1e-3) / 1e6, mflups=n_fluid * args.steps / (ms * 1e-3) / 1e6,
+        e2e_mlups=n * args.steps / t_e2e / 1e6, launches=n_launch, clocks=clocks, create_s=t_create,
+        split_ms_per_step={k: v / ks for k, v in split.items()},
+        roofline={"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                  "traffic": None, "peak_source": peak_src, "kernel": "k_fused_step" if fused else "k_collide_baseline",
+                  "bytes_per_launch": bytes_layout, "values_per_update": values,
+                  "kernel_ms": t_collide * 1e3, "kernel_share_of_step": split["collide"] / max(sum(split.values()), 1e-30),
+                  "canonical": {"bytes_per_update": 36 * rs + 1, "achieved": bytes_canon / t_collide / 1e9,
+                                "frac": bytes_canon / t_collide / 1e9 / peak,
+                                "note": "same time, counted as if all 18 N_i + 18 B_i moved (SURVEY 8(d) canonical)"}},
+        diag={"mass_drift_rel": float((dg["sum_phi"] - float(w.phi0[w.mask == 0].sum())) / max(float(w.phi0[w.mask == 0].sum()), 1e-30)),
+              "umax": dg["umax"], "nan": dg["nan"], "phi_min": dg["phi_min"], "phi_max": dg["phi_max"]},
+        h2d=n * 8, d2h=5 * n * 8, n_ghost=sim.n_ghost, workspace_gb=sim.workspace_bytes / 1e9)
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    return res
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=8192)
+    ap.add_argument("--precision", default="both", choices=["64", "32", "both"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"),
+                    help="ncu dram bytes per launch of the dominant kernel, written by hand from an ncu capture")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    from paper_2605_30878_b200 import binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the CPU oracle")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+
+    sched = {"auto": binding.SCHEDULE_AUTO, "baseline": binding.SCHEDULE_BASELINE, "fused": binding.SCHEDULE_FUSED}[args.schedule]
+    w = wl.config5(seed=rank, n=args.n)                # replicas: same recipe, rank-specific seed
+    precs = [64, 32] if args.precision == "both" else [int(args.precision)]
+    results = {p: bench_precision(args, w, p, sched, local, dist) for p in precs}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_oracle_rate(steps=10, warmup=2, budget_s=20.0)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "mflups")}
+
+    if rank == 0:
+        main_p = precs[0]
+        r = results[main_p]
+        traffic = None
+        try:
+            with open(args.traffic_json) as f:
+                tj = json.load(f)
+            key = f"{r['roofline']['kernel']}_f{main_p}_n{args.n}"
+            traffic = tj.get(key, {}).get("dram_bytes_per_launch")
+        except Exception:
+            pass
+        r["roofline"]["traffic"] = traffic
+        line = {
+            "metric": METRIC, "value": r["mlups"] * world, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": r["ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64" if main_p == 64 else "f32", "data": "synthetic",
+            "config": {"workload": f"config5 porous medium {args.n}x{args.n} periodic, random disks r~U(8,32) to porosity 0.65, "
+                                   f"liquid blobs to 50% of pore space, density ratio 1000, viscosity ratio 100, theta=110deg",
+                       "n_fluid": int(w.meta["n_fluid"]), "n_ghost": r["n_ghost"], "n_disks": int(w.meta["n_disks"]),
+                       "schedule": args.schedule, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": f"state {r['workspace_gb']:.1f} GB >> 126 MB L2 (inputs larger than L2, no flush needed)",
+                       "create_s": r["create_s"]},
+            "mflups": r["mflups"] * world,
+            "e2e": {"value": r["e2e_mlups"] * world, "unit": "MLUPS", "h2d_bytes_per_step": r["h2d"] / args.steps,
+                    "d2h_bytes_per_step": r["d2h"] / args.steps,
+                    "what": "lbm_init(host phi0) + lbm_step(K) + lbm_get(5 host fields), pinned host buffers, wall clock"},
+            "gpu_launches": r["launches"], "clocks": r["clocks"], "roofline": r["roofline"],
+            "kernel_ms_per_step": r["split_ms_per_step"], "diag": r["diag"], "cpu_baseline": cpu,
+        }
+        for p in precs[1:]:
+            q = results[p]
+            line[f"fp{p}"] = {"value": q["mlups"] * world, "mflups": q["mflups"] * world, "ms_per_step": q["ms"] / args.steps,
+                              "e2e": q["e2e_mlups"] * world, "roofline": q["roofline"], "clocks": q["clocks"],
+                              "kernel_ms_per_step": q["split_ms_per_step"], "diag": q["diag"], "gpu_launches": q["launches"]}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
