@@ -10,6 +10,7 @@
 #include "../../include/lbm.h"
 #include "lbm_fused.cuh"
 #include "lbm_kernels.cuh"
+#include "lbm_warp.cuh"
 
 using namespace lbm;
 
@@ -37,6 +38,7 @@ struct lbm_ctx {
   int ng;
   int is32;
   int fused;
+  int sched;         // resolved LBM_SCHEDULE_* (never AUTO)
   int keep_B;
   int B_valid;       // B planes of buffer `cur` hold the post-collision B* of the last step
   cudaStream_t st;
@@ -48,6 +50,7 @@ struct lbm_ctx {
   void* phi[2];
   uint8_t* cls;
   uint8_t* links;
+  uint16_t* cl16;     // class byte | link byte << 8 (WARP schedule reads one word per node)
   int* gidx;
   int* corner;
   void* wgt;
@@ -102,7 +105,7 @@ int validate(const lbm_params* P, const char** why) {
   if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
   if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
   if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
-  if (P->schedule < 0 || P->schedule > 2) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 3) { *why = "unknown schedule"; return LBM_EINVAL; }
   if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
   return LBM_OK;
 }
@@ -134,6 +137,7 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
   char* p1 = A.take<char>(n * rs);
   uint8_t* cls = A.take<uint8_t>(n);
   uint8_t* links = A.take<uint8_t>(n);
+  uint16_t* cl16 = A.take<uint16_t>(n);
   int* blk_cnt = A.take<int>(nblk);
   int* blk_off = A.take<int>(nblk);
   int* scal = A.take<int>(64);
@@ -151,7 +155,7 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
   uint8_t* csolid = A.take<uint8_t>(g);
   if (c && base) {
     c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
-    c->cls = cls; c->links = links; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
+    c->cls = cls; c->links = links; c->cl16 = cl16; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
     c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid; c->blk_cnt = blk_cnt;
     c->blk_off = blk_off; c->scal = scal; c->stage = stage; c->diag_out = diag_out;
     c->samp_idx = samp; c->samp_cap = samp_cap;
@@ -222,9 +226,14 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     c->launches[1]++;
     c->B_valid = 1;
   } else {
-    launch_fused_step<R>(C, c->cls, c->links, (const R*)c->N[c->cur], (R*)c->N[c->cur ^ 1],
-                         write_B ? (R*)c->B[0] : nullptr, (const R*)c->phi[c->pcur],
-                         (R*)c->phi[c->pcur ^ 1], c->st);
+    if (c->sched == LBM_SCHEDULE_WARP)
+      launch_fused_warp<R>(C, c->cl16, (const R*)c->N[c->cur], (R*)c->N[c->cur ^ 1],
+                           write_B ? (R*)c->B[0] : nullptr, (const R*)c->phi[c->pcur],
+                           (R*)c->phi[c->pcur ^ 1], c->st);
+    else
+      launch_fused_step<R>(C, c->cls, c->links, (const R*)c->N[c->cur], (R*)c->N[c->cur ^ 1],
+                           write_B ? (R*)c->B[0] : nullptr, (const R*)c->phi[c->pcur],
+                           (R*)c->phi[c->pcur ^ 1], c->st);
     c->cur ^= 1;
     c->pcur ^= 1;
     c->launches[0]++;
@@ -308,6 +317,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   c->n = n;
   c->is32 = prm->precision == 32;
   c->fused = use_fused(prm) ? 1 : 0;
+  c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? LBM_SCHEDULE_WARP : prm->schedule;
   c->st = (cudaStream_t)cuda_stream;
   c->Cd = make_consts<double>(*prm);
   c->Cf = make_consts<float>(*prm);
@@ -325,6 +335,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   CKC(cudaMemcpyAsync(d_mask, mask, n, cudaMemcpyHostToDevice, c->st));
   k_classify<<<nblk, 256, 0, c->st>>>(d_mask, prm->nx, prm->ny, c->cls, c->links, c->blk_cnt, nullptr);
   k_scan_blocks<<<1, 1024, 0, c->st>>>(c->blk_cnt, (int)nblk, c->blk_off, c->scal);
+  k_pack_cl16<<<nblk, 256, 0, c->st>>>(c->cls, c->links, (long long)n, c->cl16);
   CKC(cudaGetLastError());
   int ng = 0;
   CKC(cudaMemcpyAsync(&ng, c->scal, sizeof(int), cudaMemcpyDeviceToHost, c->st));

@@ -120,6 +120,14 @@ __global__ void __launch_bounds__(1024) k_scan_blocks(const int* __restrict__ cn
   if (threadIdx.x == 0) *total = carry;
 }
 
+// class byte and link byte of every node as one 16-bit word (WARP schedule)
+__global__ void __launch_bounds__(256) k_pack_cl16(const uint8_t* __restrict__ cls,
+                                                   const uint8_t* __restrict__ links, long long n,
+                                                   uint16_t* __restrict__ cl16) {
+  const long long k = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (k < n) cl16[k] = (uint16_t)(cls[k] | ((cls[k] == 1 ? links[k] : 0u) << 8));
+}
+
 // index-sorted compaction of ghost nodes
 __global__ void __launch_bounds__(256) k_compact_ghosts(const uint8_t* __restrict__ cls, long long n,
                                                         const int* __restrict__ block_off,
