@@ -3,7 +3,7 @@
 on BASELINE.json's config 5 (porous medium, density ratio 1000, theta = 110 deg) at 8192^2.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--n 8192] [--precision 64|32|both] [--schedule auto|baseline|fused|warp]
+                    [--n 8192] [--precision 64|32|both] [--schedule auto|baseline|fused|warp|pair]
 
 Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement"):
   value        MLUPS (Eq. 14: all grid nodes x steps / time / 1e6), device-resident state,
@@ -211,7 +211,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
         e2e_mlups=n * args.steps / t_e2e / 1e6, launches=n_launch, clocks=clocks, create_s=t_create,
         split_ms_per_step={k: v / ks for k, v in split.items()},
         roofline={"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                  "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_FUSED: "k_fused_step"}.get(schedule, "k_fused_warp"),
+                  "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_FUSED: "k_fused_step", binding.SCHEDULE_WARP: "k_fused_warp"}.get(schedule, "k_fused_pair"),
                   "bytes_per_launch": bytes_layout, "values_per_update": values,
                   "kernel_ms": t_collide * 1e3, "kernel_share_of_step": split["collide"] / max(sum(split.values()), 1e-30),
                   "canonical": {"bytes_per_update": 36 * rs + 1, "achieved": bytes_canon / t_collide / 1e9,
@@ -234,7 +234,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=8192)
     ap.add_argument("--precision", default="both", choices=["64", "32", "both"])
-    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "warp"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "warp", "pair"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"),
                     help="ncu dram bytes per launch of the dominant kernel, written by hand from an ncu capture")
@@ -261,7 +261,7 @@ def main():
         dist = dist_mod
 
     sched = {"auto": binding.SCHEDULE_AUTO, "baseline": binding.SCHEDULE_BASELINE, "fused": binding.SCHEDULE_FUSED,
-             "warp": binding.SCHEDULE_WARP}[args.schedule]
+             "warp": binding.SCHEDULE_WARP, "pair": binding.SCHEDULE_PAIR}[args.schedule]
     w = wl.config5(seed=rank, n=args.n)                # replicas: same recipe, rank-specific seed
     precs = [64, 32] if args.precision == "both" else [int(args.precision)]
     results = {p: bench_precision(args, w, p, sched, local, dist) for p in precs}

@@ -49,13 +49,17 @@ enum { LBM_FLUID_BULK = 0, LBM_FLUID_BOUNDARY = 1, LBM_GHOST = 2, LBM_SOLID_BULK
 
 /* launch schedules of lbm_step (same arithmetic per node, different kernel decomposition) */
 enum {
-  LBM_SCHEDULE_AUTO = 0,      /* the fastest schedule available (currently WARP)                  */
+  LBM_SCHEDULE_AUTO = 0,      /* the fastest schedule available (currently PAIR)                  */
   LBM_SCHEDULE_BASELINE = 1,  /* 3 launches/step: collide+stream, phi = sum B, ghost; N and B in HBM */
   LBM_SCHEDULE_FUSED = 2,     /* 2 launches/step: tiled collide+stream that also produces phi(t+1)
                                  from B* held in shared memory (B never touches HBM), ghost        */
-  LBM_SCHEDULE_WARP = 3       /* 2 launches/step like FUSED but barrier-free: one warp marches down a
+  LBM_SCHEDULE_WARP = 3,      /* 2 launches/step like FUSED but barrier-free: one warp marches down a
                                  30-column strip, phi(t+1) is assembled in registers by warp
-                                 shuffles, loads are software-pipelined one row ahead              */
+                                 shuffles, loads run ahead through a per-warp cp.async ring        */
+  LBM_SCHEDULE_PAIR = 4       /* like WARP, but every lane owns an aligned pair of nodes: each
+                                 population is fetched once, unshifted, as an 8/16-byte vector;
+                                 propagation in x is a warp shuffle; fp32 arithmetic is packed
+                                 (FFMA2).  Needs even nx, else FUSED is used                        */
 };
 
 typedef struct lbm_ctx lbm_ctx;                 /* opaque; one simulation                         */

@@ -19,7 +19,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 _SO = os.path.join(_HERE, "liblbm_b200.so")
 
-SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_WARP = 0, 1, 2, 3
+SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_WARP, SCHEDULE_PAIR = 0, 1, 2, 3, 4
 FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
 EXPORTS = ("lbm_plan", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
@@ -44,6 +44,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
                "-shared", "-Xcompiler", "-fPIC", "-diag-suppress", "550", "-o", _SO,
                os.path.join(_CSRC, "lbm_api.cu")]
+        cmd[1:1] = os.environ.get("LBM_NVCC_EXTRA", "").split()   # tuning sweeps: -DLBM_PAIR_DP32=1 ...
         if verbose:
             cmd.insert(1, "-Xptxas")
             cmd.insert(2, "-v")

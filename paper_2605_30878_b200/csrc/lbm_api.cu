@@ -10,6 +10,7 @@
 #include "../../include/lbm.h"
 #include "lbm_fused.cuh"
 #include "lbm_kernels.cuh"
+#include "lbm_pair.cuh"
 #include "lbm_warp.cuh"
 
 using namespace lbm;
@@ -96,7 +97,7 @@ int validate(const lbm_params* P, const char** why) {
   *why = "";
   if (!P) { *why = "null params"; return LBM_EINVAL; }
   if (P->nx < 3 || P->ny < 3) { *why = "nx, ny must be >= 3"; return LBM_EINVAL; }
-  if ((long long)P->nx * P->ny > 0x7fffffffLL / 2) { *why = "nx*ny too large for 32-bit indices"; return LBM_EINVAL; }
+  if ((long long)P->nx * P->ny > 0xffffffffLL / 9 - 4096) { *why = "nx*ny too large: 9 nx ny must fit 32-bit element offsets"; return LBM_EINVAL; }
   if (P->precision != 32 && P->precision != 64) { *why = "precision must be 32 or 64"; return LBM_EINVAL; }
   if (!(P->rho_l > 0.0) || !(P->rho_g > 0.0)) { *why = "densities must be > 0"; return LBM_EINVAL; }
   if (!(P->nu_l > 0.0) || !(P->nu_g > 0.0)) { *why = "viscosities must be > 0 (tau > 1/2)"; return LBM_EINVAL; }
@@ -105,7 +106,7 @@ int validate(const lbm_params* P, const char** why) {
   if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
   if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
   if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
-  if (P->schedule < 0 || P->schedule > 3) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 4) { *why = "unknown schedule"; return LBM_EINVAL; }
   if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
   return LBM_OK;
 }
@@ -115,6 +116,13 @@ int check_walls(const lbm_params* P, const uint8_t* mask) {
   for (int i = 0; i < P->nx; i++)
     if (!mask[i] || !mask[(size_t)(P->ny - 1) * P->nx + i]) return LBM_EINVAL;
   return LBM_OK;
+}
+
+// element stride between population planes: nx*ny rounded up to 64 elements plus 37*64, so that
+// plane strides are never a power of two (8192^2 planes would otherwise all map to the same L2 sets)
+size_t plane_stride(const lbm_params* P) {
+  const size_t n = (size_t)P->nx * P->ny;
+  return ((n + 63) & ~(size_t)63) + 37 * 64;
 }
 
 bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELINE; }
@@ -129,15 +137,16 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
   const size_t nblk = (n + 255) / 256;
   const bool fused = use_fused(P);
   Arena A{base, 0};
-  char* N0 = A.take<char>(9 * n * rs);
-  char* N1 = A.take<char>(9 * n * rs);
-  char* B0 = A.take<char>(9 * n * rs);
-  char* B1 = fused ? nullptr : A.take<char>(9 * n * rs);
+  const size_t ps = plane_stride(P);
+  char* N0 = A.take<char>(9 * ps * rs);
+  char* N1 = A.take<char>(9 * ps * rs);
+  char* B0 = A.take<char>(9 * ps * rs);
+  char* B1 = fused ? nullptr : A.take<char>(9 * ps * rs);
   char* p0 = A.take<char>(n * rs);
   char* p1 = A.take<char>(n * rs);
   uint8_t* cls = A.take<uint8_t>(n);
   uint8_t* links = A.take<uint8_t>(n);
-  uint16_t* cl16 = A.take<uint16_t>(n);
+  uint16_t* cl16 = A.take<uint16_t>(n + 2);   // +2: the WARP kernel copies aligned 4-byte pairs
   int* blk_cnt = A.take<int>(nblk);
   int* blk_off = A.take<int>(nblk);
   int* scal = A.take<int>(64);
@@ -170,6 +179,7 @@ Consts<R> make_consts(const lbm_params& P) {
   const double ct = cos(P.theta_deg * M_PI / 180.0);
   const double eps = -(4.0 / P.W) * ct;                 // Eq. 9 (:80), dx = 1
   C.nx = P.nx; C.ny = P.ny;
+  C.ps = plane_stride(&P);
   C.rho_g = (R)P.rho_g; C.drho = (R)(P.rho_l - P.rho_g);
   C.inu_g = (R)(1.0 / P.nu_g); C.dinu = (R)(1.0 / P.nu_l - 1.0 / P.nu_g);
   C.s48W = (R)(P.sigma * 48.0 / P.W); C.s15W = (R)(P.sigma * 1.5 * P.W);
@@ -226,14 +236,15 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     c->launches[1]++;
     c->B_valid = 1;
   } else {
-    if (c->sched == LBM_SCHEDULE_WARP)
-      launch_fused_warp<R>(C, c->cl16, (const R*)c->N[c->cur], (R*)c->N[c->cur ^ 1],
-                           write_B ? (R*)c->B[0] : nullptr, (const R*)c->phi[c->pcur],
-                           (R*)c->phi[c->pcur ^ 1], c->st);
-    else
-      launch_fused_step<R>(C, c->cls, c->links, (const R*)c->N[c->cur], (R*)c->N[c->cur ^ 1],
-                           write_B ? (R*)c->B[0] : nullptr, (const R*)c->phi[c->pcur],
-                           (R*)c->phi[c->pcur ^ 1], c->st);
+    const R* Ns = (const R*)c->N[c->cur];
+    R* Nd = (R*)c->N[c->cur ^ 1];
+    R* Bd = write_B ? (R*)c->B[0] : nullptr;
+    const R* pi = (const R*)c->phi[c->pcur];
+    R* po = (R*)c->phi[c->pcur ^ 1];
+    bool done = false;
+    if (c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair<R>(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
+    if (!done && c->sched == LBM_SCHEDULE_WARP) done = launch_fused_warp<R>(C, c->cl16, Ns, Nd, Bd, pi, po, c->st) == 0;
+    if (!done) launch_fused_step<R>(C, c->cls, c->links, Ns, Nd, Bd, pi, po, c->st);
     c->cur ^= 1;
     c->pcur ^= 1;
     c->launches[0]++;
@@ -317,7 +328,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   c->n = n;
   c->is32 = prm->precision == 32;
   c->fused = use_fused(prm) ? 1 : 0;
-  c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? LBM_SCHEDULE_WARP : prm->schedule;
+  c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? LBM_SCHEDULE_PAIR : prm->schedule;
   c->st = (cudaStream_t)cuda_stream;
   c->Cd = make_consts<double>(*prm);
   c->Cf = make_consts<float>(*prm);

@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(TX) k_fused_step(const Consts<R> C, const uint
   R(*sB)[9][TX] = reinterpret_cast<R(*)[9][TX]>(smem_raw);   // [4][9][TX]
 
   const int nx = C.nx, ny = C.ny;
-  const size_t n = (size_t)nx * ny;
+  const size_t n = C.ps;   // plane stride
   const int tx = threadIdx.x;
   const int x0 = blockIdx.x * (TX - 2);
   const int j0 = blockIdx.y * TY;

@@ -1,7 +1,7 @@
 // lbm_kernels.cuh — CUDA kernels of liblbm_b200 (sm_100a).  See DESIGN.md "Kernels".
 //
 // State layout in HBM (structure of arrays, x fastest, idx = j*nx + i):
-//   pop[q*n + idx]  post-COLLISION deviations n_q* = N_q* - chi_q of the last step, stored at the
+//   pop[q*ps + idx] (ps = padded plane stride, Consts::ps) post-COLLISION deviations n_q* = N_q* - chi_q of the last step, stored at the
 //                   node that produced them; propagation (A16-A17) is the pull on the next read:
 //                   N_q(x, t+1) = N_q*(x - c_q, t), or N_opp(q)*(x, t) if x - c_q is solid
 //                   (half-way bounce-back, R12).  Double-buffered.
@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(256) k_collide_baseline(const Consts<R> C,
                                                           const R* __restrict__ phi) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
-  const size_t n = (size_t)C.nx * C.ny;
+  const size_t n = C.ps;   // plane stride
   const int k = j * C.nx + i;
   const uint8_t c = cls[k];
   if (c >= 2) return;
@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(256) k_phi_sum(const Consts<R> C, const uint8_
                                                  const R* __restrict__ Bsrc, R* __restrict__ phi) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
-  const size_t n = (size_t)C.nx * C.ny;
+  const size_t n = C.ps;   // plane stride
   const int k = j * C.nx + i;
   const uint8_t c = cls[k];
   if (c >= 2) return;
@@ -343,7 +343,7 @@ __global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* 
                                               R* __restrict__ phiB) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
-  const size_t n = (size_t)C.nx * C.ny;
+  const size_t n = C.ps;   // plane stride
   const int k = j * C.nx + i;
   const uint8_t c = cls[k];
   if (c >= 2) {
@@ -367,12 +367,12 @@ __global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* 
     const bool blocked = q > 0 && ((lk >> (oq - 1)) & 1u);
     const int src = blocked ? k : b.dst[q];
     const int qq = blocked ? oq : q;
-    const R ux = u0 ? (R)u0[src] : R(0), uy = u0 ? (R)u0[n + src] : R(0);
+    const R ux = u0 ? (R)u0[src] : R(0), uy = u0 ? (R)u0[(size_t)C.nx * C.ny + src] : R(0);
     const R dev = neq_dev_p0<R>(qq, ux, uy);
     Npop[q * n + k] = dev;
     if (Bpop) Bpop[q * n + k] = (R)phi0[src] * (chi[qq] + dev);
     // phi(x, 0) = sum_i B_i(x, 0) = sum_i phi0(x) N_i^eq(u0(x)) in the oracle's order (A13)
-    const R uxk = u0 ? (R)u0[k] : R(0), uyk = u0 ? (R)u0[n + k] : R(0);
+    const R uxk = u0 ? (R)u0[k] : R(0), uyk = u0 ? (R)u0[(size_t)C.nx * C.ny + k] : R(0);
     s += (R)phi0[k] * (chi[q] + neq_dev_p0<R>(q, uxk, uyk));
   }
   phiA[k] = s;
@@ -391,7 +391,7 @@ __global__ void __launch_bounds__(256) k_moments(const Consts<R> C, const uint8_
                                                  double* __restrict__ o_p) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
-  const size_t n = (size_t)C.nx * C.ny;
+  const size_t n = C.ps;   // plane stride
   const int k = j * C.nx + i;
   const uint8_t c = cls[k];
   if (o_phi) o_phi[k] = (double)phi[k];
@@ -423,7 +423,7 @@ __global__ void __launch_bounds__(256) k_gather_plane(const Consts<R> C, const u
                                                       double* __restrict__ out) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
-  const size_t n = (size_t)C.nx * C.ny;
+  const size_t n = C.ps;   // plane stride
   const int k = j * C.nx + i;
   const uint8_t c = cls[k];
   if (c >= 2) { out[k] = 0.0; return; }
@@ -444,7 +444,7 @@ __global__ void __launch_bounds__(128) k_gather_samples(const Consts<R> C, const
                                                         double* __restrict__ out) {
   const long long t = (long long)blockIdx.x * 128 + threadIdx.x;
   if (t >= m) return;
-  const size_t n = (size_t)C.nx * C.ny;
+  const size_t n = C.ps;   // plane stride
   const int k = (int)idx[t];
   const uint8_t c = cls[k];
   const Nbr b = make_nbr(k % C.nx, k / C.nx, C.nx, C.ny);
@@ -514,7 +514,7 @@ __global__ void __launch_bounds__(256) k_diag_partial(const Consts<R> C, const u
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   DiagVec v = diag_identity();
   if (i < C.nx) {
-    const size_t n = (size_t)C.nx * C.ny;
+    const size_t n = C.ps;   // plane stride
     const int k = j * C.nx + i;
     const uint8_t c = cls[k];
     if (c < 2) {

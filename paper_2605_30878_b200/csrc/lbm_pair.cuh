@@ -1,0 +1,354 @@
+// lbm_pair.cuh — PAIR schedule: the fused pull-stream + collide + segregation + phi(t+1) kernel in
+// which every lane owns TWO x-adjacent nodes (an aligned pair), every value moves as an aligned
+// 8-byte (fp32) or 16-byte (fp64) vector, and fp32 arithmetic is packed (FFMA2/FADD2/FMUL2).
+// Same arithmetic per node as the other schedules (node_update_t), same HBM state.
+//
+//   * a warp owns a strip of 64 columns [60 g - 2, 60 g + 62): 60 output columns and two halo
+//     columns per side (one is needed; pairs must stay aligned), and marches down TY rows (+1 halo
+//     row per end).  No shared data between warps, no block barrier.
+//   * every population is fetched from HBM exactly once per strip, UNSHIFTED, at its own node, by
+//     cp.async (LDGSTS) into a private shared-memory ring DP+1 rows ahead of the collision; pairs
+//     with no fluid node are not fetched.  Propagation (A16-A17, :318-322) is done on chip: the row
+//     part by reading the ring slot of the neighbouring row, the column part by one warp shuffle
+//     per shifted plane.  Half-way bounce-back (R12) selects the node's own opposite population,
+//     which is already on chip.
+//   * phi(x, t+1) = sum_q B_q*(x - c_q, t) (A13) is assembled in registers as in lbm_warp.cuh.
+//   * stores are aligned vectors at the node's own position.
+#pragma once
+#include "lbm_kernels.cuh"
+#include "lbm_warp.cuh"   // cp_async_commit / cp_async_wait
+
+namespace lbm {
+
+// pipeline depth and CTA shape per precision (overridable at build time for tuning sweeps)
+#ifndef LBM_PAIR_DP32
+#define LBM_PAIR_DP32 2
+#endif
+#ifndef LBM_PAIR_DP64
+#define LBM_PAIR_DP64 1
+#endif
+#ifndef LBM_PAIR_MINB32
+#define LBM_PAIR_MINB32 4
+#endif
+#ifndef LBM_PAIR_MINB64
+#define LBM_PAIR_MINB64 2
+#endif
+#ifndef LBM_PAIR_WARPS
+#define LBM_PAIR_WARPS 4
+#endif
+#ifndef LBM_PAIR_FULLSECTOR
+#define LBM_PAIR_FULLSECTOR 1
+#endif
+#ifndef LBM_PAIR_TY
+#define LBM_PAIR_TY 64
+#endif
+
+// ---- pair value types ----
+struct __align__(16) D2 {   // two fp64 nodes; arithmetic is done node by node (no packed fp64 instructions)
+  double x, y;
+};
+template <typename R> struct PairOf;
+template <> struct PairOf<float> { using type = F2; };
+template <> struct PairOf<double> { using type = D2; };
+
+__device__ __forceinline__ float lo(F2 a) { return a.v.x; }
+__device__ __forceinline__ float hi(F2 a) { return a.v.y; }
+__device__ __forceinline__ double lo(D2 a) { return a.x; }
+__device__ __forceinline__ double hi(D2 a) { return a.y; }
+__device__ __forceinline__ F2 mk(float a, float b) { return f2(a, b); }
+__device__ __forceinline__ D2 mk(double a, double b) { return D2{a, b}; }
+__device__ __forceinline__ D2 operator+(D2 a, D2 b) { return D2{a.x + b.x, a.y + b.y}; }
+
+// propagation in x: value arriving from the left neighbour (c_x = +1) / right neighbour (c_x = -1)
+template <typename V>
+__device__ __forceinline__ V from_left(V a) {
+  return mk(__shfl_up_sync(0xffffffffu, hi(a), 1), lo(a));
+}
+template <typename V>
+__device__ __forceinline__ V from_right(V a) {
+  return mk(hi(a), __shfl_down_sync(0xffffffffu, lo(a), 1));
+}
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async_vec(unsigned saddr, const void* gptr) {
+  // .ca for every size: with .cg (L1 bypass) the two 16-byte lanes of a sector each fetch it from L2
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(saddr), "l"(gptr), "n"(BYTES) : "memory");
+}
+
+// shared-memory ring of one warp: row stages hold the own-position populations and phi of the 64
+// columns; class stages the packed class words (two 16-bit words per lane)
+template <typename R, int DP>
+struct PairRing {
+  using V = typename PairOf<R>::type;
+  static constexpr int NS = DP + 2;        // rows i .. i+1+DP
+  static constexpr int CS = 2 * DP + 2;    // class rows i .. i+1+2DP
+  V N[NS][9][32];
+  V P[NS][32];
+  unsigned Cw[CS][32];
+};
+
+// collide the two nodes of a pair; fa/fb: node is fluid.  fp32: packed, masked; fp64: node by node
+__device__ __forceinline__ void collide_pair(const Consts<float>& C, const F2 (&n)[9], const F2 (&ph)[9],
+                                             bool fa, bool fb, F2 (&ns)[9], F2 (&bs)[9]) {
+  node_update_t<F2, float, true, true>(C, n, ph, ns, bs, nullptr, f2(fa ? 1.0f : 0.0f, fb ? 1.0f : 0.0f));
+  if (!(fa && fb)) {   // the solid partner stores zeros, so that its slots stay finite
+#pragma unroll
+    for (int q = 0; q < 9; q++) ns[q] = f2(fa ? ns[q].v.x : 0.0f, fb ? ns[q].v.y : 0.0f);
+  }
+}
+__device__ __forceinline__ void collide_pair(const Consts<double>& C, const D2 (&n)[9], const D2 (&ph)[9],
+                                             bool fa, bool fb, D2 (&ns)[9], D2 (&bs)[9]) {
+#pragma unroll
+  for (int q = 0; q < 9; q++) ns[q] = bs[q] = D2{0.0, 0.0};
+  if (fa) {
+    double n1[9], p1[9], s1[9], b1[9];
+#pragma unroll
+    for (int q = 0; q < 9; q++) { n1[q] = n[q].x; p1[q] = ph[q].x; }
+    node_update<double, true>(C, n1, p1, s1, b1, nullptr);
+#pragma unroll
+    for (int q = 0; q < 9; q++) { ns[q].x = s1[q]; bs[q].x = b1[q]; }
+  }
+  if (fb) {
+    double n1[9], p1[9], s1[9], b1[9];
+#pragma unroll
+    for (int q = 0; q < 9; q++) { n1[q] = n[q].y; p1[q] = ph[q].y; }
+    node_update<double, true>(C, n1, p1, s1, b1, nullptr);
+#pragma unroll
+    for (int q = 0; q < 9; q++) { ns[q].y = s1[q]; bs[q].y = b1[q]; }
+  }
+}
+
+template <typename R, int DP, int WARPS, int MINB, bool WRITE_B>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
+    k_fused_pair(const Consts<R> C, const uint16_t* __restrict__ cl16, const R* __restrict__ Nsrc,
+                 R* __restrict__ Ndst, R* __restrict__ Bdst, const R* __restrict__ phi_in,
+                 R* __restrict__ phi_out, int TY) {
+  using Ring = PairRing<R, DP>;
+  using V = typename PairOf<R>::type;
+  constexpr unsigned FULL = 0xffffffffu;
+  constexpr int VB = 2 * (int)sizeof(R);   // bytes of a pair
+  constexpr int NS = Ring::NS, CS = Ring::CS;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Ring& S = reinterpret_cast<Ring*>(smem_raw)[threadIdx.x >> 5];
+  const int lane = threadIdx.x & 31;
+  const unsigned sN0 = (unsigned)__cvta_generic_to_shared(&S.N[0][0][lane]);
+  const unsigned sP0 = (unsigned)__cvta_generic_to_shared(&S.P[0][lane]);
+  const unsigned sC0 = (unsigned)__cvta_generic_to_shared(&S.Cw[0][lane]);
+  constexpr unsigned N_STAGE = 9 * 32 * VB, N_PLANE = 32 * VB, P_STAGE = 32 * VB, C_STAGE = 32 * 4;
+
+  const int nx = C.nx, ny = C.ny;   // nx is even (checked by the launcher)
+  const unsigned ps = (unsigned)C.ps;
+  const int g = blockIdx.x * WARPS + (threadIdx.x >> 5);
+  if (60 * g >= nx) return;                              // whole warp; the kernel has no block barrier
+  const int xend = min(60 * g + 60, nx);                 // one past the last output column (even)
+  const int lxa = 60 * g - 2 + 2 * lane;                 // logical column of the pair's first node
+  const bool col_out = lane >= 1 && lane <= 30 && lxa < xend;
+  int xa = lxa % nx;                                     // every lane is a valid periodic pair
+  if (xa < 0) xa += nx;
+  // lanes whose pairs share a 32-byte sector of a population plane (rows keep the sector phase only
+  // if the row pitch is a multiple of 32 bytes); a sector that holds any fluid node is stored whole
+  // (zeros on its solid nodes), so that HBM never has to read-modify-write a partial sector
+  const int sector = (lxa + 64) * (int)sizeof(R) / 32;
+  const unsigned gmask = (LBM_PAIR_FULLSECTOR && (nx * (int)sizeof(R)) % 32 == 0) ? __match_any_sync(FULL, sector) : (1u << lane);
+  const int j0 = blockIdx.y * TY;
+  const int rows = min(TY, ny - j0);
+  const int last = rows + 1;                             // march row m = grid row j0-1+m; collided: 0..last
+
+  auto rowoff = [=](int m) -> unsigned {                 // element offset of march row m, periodic in y
+    int r = j0 - 1 + m;
+    r = r < 0 ? r + ny : (r >= ny ? r - ny : r);
+    return (unsigned)r * (unsigned)nx;
+  };
+  auto slotN = [](int m) { return (m + 1) % NS; };
+  auto slotC = [](int m) { return (m + 1) % CS; };
+  // ---- asynchronous fetches ----
+  auto issue_cls = [&](int m) {   // the two class words of the pair (one aligned 4-byte word)
+    cp_async_vec<4>(sC0 + (unsigned)slotC(m) * C_STAGE, cl16 + (rowoff(m) + (unsigned)xa));
+  };
+  auto issue_row = [&](int m) {   // own-position populations and phi of march row m
+    const unsigned w2 = S.Cw[slotC(m)][lane];
+    const unsigned ca = w2 & 0xffu, cb = (w2 >> 16) & 0xffu;
+    const unsigned k = rowoff(m) + (unsigned)xa;
+    const int sl = slotN(m);
+    if (ca != 3u || cb != 3u) cp_async_vec<VB>(sP0 + (unsigned)sl * P_STAGE, phi_in + k);
+    if (ca < 2u || cb < 2u) {
+      const unsigned d = sN0 + (unsigned)sl * N_STAGE;
+      const bool lower = m >= 0, upper = m <= last;      // row -1 feeds only c_y = +1, row last+1 only c_y = -1
+      if (lower && upper) {
+        cp_async_vec<VB>(d + 0 * N_PLANE, Nsrc + k);
+        cp_async_vec<VB>(d + 1 * N_PLANE, Nsrc + (1u * ps + k));
+        cp_async_vec<VB>(d + 3 * N_PLANE, Nsrc + (3u * ps + k));
+      }
+      if (upper) {
+        cp_async_vec<VB>(d + 2 * N_PLANE, Nsrc + (2u * ps + k));
+        cp_async_vec<VB>(d + 5 * N_PLANE, Nsrc + (5u * ps + k));
+        cp_async_vec<VB>(d + 6 * N_PLANE, Nsrc + (6u * ps + k));
+      }
+      if (lower) {
+        cp_async_vec<VB>(d + 4 * N_PLANE, Nsrc + (4u * ps + k));
+        cp_async_vec<VB>(d + 7 * N_PLANE, Nsrc + (7u * ps + k));
+        cp_async_vec<VB>(d + 8 * N_PLANE, Nsrc + (8u * ps + k));
+      }
+    }
+  };
+
+  // ---- prologue ----
+  {   // stale ring entries are read (and discarded) for solid nodes: they must be finite
+    const V z = mk(R(0), R(0));
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
+#pragma unroll
+      for (int q = 0; q < 9; q++) S.N[s][q][lane] = z;
+      S.P[s][lane] = z;
+    }
+  }
+  for (int m = -1; m <= 2 * DP; m++)
+    if (m <= last + 1) issue_cls(m);
+  cp_async_commit();
+  cp_async_wait<0>();
+  for (int m = -1; m <= DP; m++) {
+    if (m <= last + 1) issue_row(m);
+    cp_async_commit();
+  }
+  cp_async_wait<DP - 1>();   // rows -1, 0, 1 have landed
+
+  // carried between iterations (iteration i collides march row i)
+  V Bprev[3], Ccur[3];       // planes 2,5,6 of row i-1; planes 4,7,8 of row i
+  V phS[3], phC[3];          // phi of rows i-1 and i as (west, centre, east) vectors
+  {
+    const int sm1 = slotN(-1), s0 = slotN(0);
+    Bprev[0] = S.N[sm1][2][lane]; Bprev[1] = S.N[sm1][5][lane]; Bprev[2] = S.N[sm1][6][lane];
+    Ccur[0] = S.N[s0][4][lane]; Ccur[1] = S.N[s0][7][lane]; Ccur[2] = S.N[s0][8][lane];
+    const V a = S.P[sm1][lane], b = S.P[s0][lane];
+    phS[0] = from_left(a); phS[1] = a; phS[2] = from_right(a);
+    phC[0] = from_left(b); phC[1] = b; phC[2] = from_right(b);
+  }
+  unsigned kout = (unsigned)(j0 - 1) * (unsigned)nx + (unsigned)xa;   // own pair of march row i (1 <= i <= rows)
+  const V zero = mk(R(0), R(0));
+  V acc_prev = zero, up_prev = zero;
+  bool fa_prev = false, fb_prev = false;
+
+  for (int i = 0; i <= last; i++) {
+    if (i > 0) cp_async_wait<DP - 1>();   // row i+1 and the class words of row i+1+DP have landed
+    // ---- issue: populations and phi of row i+1+DP, class words of row i+1+2DP ----
+    if (i + 1 + DP <= last + 1) issue_row(i + 1 + DP);
+    if (i + 1 + 2 * DP <= last + 1) issue_cls(i + 1 + 2 * DP);
+    cp_async_commit();
+
+    // ---- on-chip operands of march row i ----
+    const int si = slotN(i), sn = slotN(i + 1);
+    const unsigned w2 = S.Cw[slotC(i)][lane];
+    const V A0 = S.N[si][0][lane], A1 = S.N[si][1][lane], A3 = S.N[si][3][lane];
+    V Bcur[3], Cnext[3];
+    Bcur[0] = S.N[si][2][lane]; Bcur[1] = S.N[si][5][lane]; Bcur[2] = S.N[si][6][lane];
+    Cnext[0] = S.N[sn][4][lane]; Cnext[1] = S.N[sn][7][lane]; Cnext[2] = S.N[sn][8][lane];
+    V phN[3];
+    phN[1] = S.P[sn][lane]; phN[0] = from_left(phN[1]); phN[2] = from_right(phN[1]);
+
+    const bool fa = (w2 & 0xffu) < 2u, fb = ((w2 >> 16) & 0xffu) < 2u;
+    const unsigned lka = fa ? (w2 >> 8) & 0xffu : 0u, lkb = fb ? (w2 >> 24) : 0u;
+    const bool any_link = __any_sync(FULL, (lka | lkb) != 0u);
+
+    // pulled populations: propagation A16-A17 on chip
+    V nn[9];
+    nn[0] = A0;       nn[1] = from_left(A1);       nn[3] = from_right(A3);
+    nn[2] = Bprev[0]; nn[5] = from_left(Bprev[1]); nn[6] = from_right(Bprev[2]);
+    nn[4] = Cnext[0]; nn[7] = from_right(Cnext[1]); nn[8] = from_left(Cnext[2]);
+    if (any_link) {   // warp-uniform; half-way bounce-back (R12): own opposite population, same row
+      const V own[9] = {A0, A1, Bcur[0], A3, Ccur[0], Bcur[1], Bcur[2], Ccur[1], Ccur[2]};   // plane q at (x, i)
+#pragma unroll
+      for (int q = 1; q < 9; q++) {
+        const V o = own[opp(q)];
+        R a = lo(nn[q]), b = hi(nn[q]);
+        if ((lka >> (q - 1)) & 1u) a = lo(o);
+        if ((lkb >> (q - 1)) & 1u) b = hi(o);
+        nn[q] = mk(a, b);
+      }
+    }
+
+    V ns[9], bs[9];
+    V bb = zero;
+    if (fa || fb) {
+      const V ph[9] = {phC[1], phC[2], phN[1], phC[0], phS[1], phN[2], phN[0], phS[0], phS[2]};
+      collide_pair(C, nn, ph, fa, fb, ns, bs);
+      if (lka | lkb) {   // link q hands the node its own B_opp(q)* back
+        R ba = R(0), bbv = R(0);
+#pragma unroll
+        for (int q = 1; q < 9; q++) {
+          if ((lka >> (q - 1)) & 1u) ba += lo(bs[opp(q)]);
+          if ((lkb >> (q - 1)) & 1u) bbv += hi(bs[opp(q)]);
+        }
+        bb = mk(ba, bbv);
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < 9; q++) ns[q] = bs[q] = zero;
+    }
+    {
+      const bool row_out = i >= 1 && i <= rows;
+      const unsigned fmask = __ballot_sync(FULL, col_out && (fa || fb));
+      if (row_out && col_out && (fmask & gmask) != 0u) {
+#pragma unroll
+        for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(Ndst + ((unsigned)q * ps + kout)) = ns[q];
+        if (WRITE_B) {
+#pragma unroll
+          for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(Bdst + ((unsigned)q * ps + kout)) = bs[q];
+        }
+      }
+    }
+    // contributions of row i to phi(t+1) of rows i-1 (down), i (mid), i+1 (up)
+    const V mid = bs[0] + from_left(bs[1]) + from_right(bs[3]);
+    const V upw = bs[2] + from_left(bs[5]) + from_right(bs[6]);
+    const V down = bs[4] + from_right(bs[7]) + from_left(bs[8]);
+    if (i >= 2 && col_out) {
+      const V pn = acc_prev + down;
+      R* dst = phi_out + (kout - (unsigned)nx);
+      if (fa_prev && fb_prev) *reinterpret_cast<V*>(dst) = pn;
+      else {
+        if (fa_prev) dst[0] = lo(pn);
+        if (fb_prev) dst[1] = hi(pn);
+      }
+    }
+    acc_prev = (up_prev + mid) + bb;
+    up_prev = upw;
+    fa_prev = fa; fb_prev = fb;
+
+    kout += (unsigned)nx;
+#pragma unroll
+    for (int t = 0; t < 3; t++) { Bprev[t] = Bcur[t]; Ccur[t] = Cnext[t]; phS[t] = phC[t]; phC[t] = phN[t]; }
+  }
+  cp_async_wait<0>();
+}
+
+template <typename R>
+struct PairCfg {
+  static constexpr int DP = sizeof(R) == 8 ? LBM_PAIR_DP64 : LBM_PAIR_DP32;
+  static constexpr int WARPS = LBM_PAIR_WARPS;
+  static constexpr int MINB = sizeof(R) == 8 ? LBM_PAIR_MINB64 : LBM_PAIR_MINB32;
+};
+
+// returns false if the grid does not fit the schedule (odd nx): the caller uses another schedule
+template <typename R>
+bool launch_fused_pair(const Consts<R>& C, const uint16_t* cl16, const R* Nsrc, R* Ndst, R* Bdst,
+                       const R* phi_in, R* phi_out, cudaStream_t st) {
+  using Cfg = PairCfg<R>;
+  constexpr int DP = Cfg::DP, WARPS = Cfg::WARPS, MINB = Cfg::MINB;
+  if (C.nx & 1) return false;
+  const int nwx = (C.nx + 59) / 60;
+  const int gx = (nwx + WARPS - 1) / WARPS;
+  // rows per warp march: long marches amortise the halo rows; small grids need enough CTAs
+  int TY = LBM_PAIR_TY;
+  while (TY > 8 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 8) TY >>= 1;
+  const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
+  const size_t smem = sizeof(PairRing<R, DP>) * WARPS;
+  auto kern = Bdst ? k_fused_pair<R, DP, WARPS, MINB, true> : k_fused_pair<R, DP, WARPS, MINB, false>;
+  static bool attr_set[2] = {false, false};
+  if (!attr_set[Bdst ? 1 : 0]) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+    attr_set[Bdst ? 1 : 0] = true;
+  }
+  kern<<<grid, 32 * WARPS, smem, st>>>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, TY);
+  return true;
+}
+
+}  // namespace lbm
