@@ -22,7 +22,7 @@ namespace lbm {
 
 // pipeline depth and CTA shape per precision (overridable at build time for tuning sweeps)
 #ifndef LBM_PAIR_DP32
-#define LBM_PAIR_DP32 2
+#define LBM_PAIR_DP32 1
 #endif
 #ifndef LBM_PAIR_DP64
 #define LBM_PAIR_DP64 1
@@ -31,7 +31,7 @@ namespace lbm {
 #define LBM_PAIR_MINB32 4
 #endif
 #ifndef LBM_PAIR_MINB64
-#define LBM_PAIR_MINB64 2
+#define LBM_PAIR_MINB64 3
 #endif
 #ifndef LBM_PAIR_WARPS
 #define LBM_PAIR_WARPS 4
@@ -58,6 +58,17 @@ __device__ __forceinline__ double hi(D2 a) { return a.y; }
 __device__ __forceinline__ F2 mk(float a, float b) { return f2(a, b); }
 __device__ __forceinline__ D2 mk(double a, double b) { return D2{a, b}; }
 __device__ __forceinline__ D2 operator+(D2 a, D2 b) { return D2{a.x + b.x, a.y + b.y}; }
+__device__ __forceinline__ D2 operator-(D2 a, D2 b) { return D2{a.x - b.x, a.y - b.y}; }
+__device__ __forceinline__ D2 operator*(D2 a, D2 b) { return D2{a.x * b.x, a.y * b.y}; }
+__device__ __forceinline__ D2 operator-(D2 a) { return D2{-a.x, -a.y}; }
+__device__ __forceinline__ D2 operator+(D2 a, double b) { return D2{a.x + b, a.y + b}; }
+__device__ __forceinline__ D2 operator+(double a, D2 b) { return D2{a + b.x, a + b.y}; }
+__device__ __forceinline__ D2 operator-(D2 a, double b) { return D2{a.x - b, a.y - b}; }
+__device__ __forceinline__ D2 operator-(double a, D2 b) { return D2{a - b.x, a - b.y}; }
+__device__ __forceinline__ D2 operator*(D2 a, double b) { return D2{a.x * b, a.y * b}; }
+__device__ __forceinline__ D2 operator*(double a, D2 b) { return D2{a * b.x, a * b.y}; }
+__device__ __forceinline__ D2 rcp_(D2 a) { return D2{1.0 / a.x, 1.0 / a.y}; }
+__device__ __forceinline__ D2 rsqrt0_(D2 a) { return D2{rsqrt0_(a.x), rsqrt0_(a.y)}; }
 
 // propagation in x: value arriving from the left neighbour (c_x = +1) / right neighbour (c_x = -1)
 template <typename V>
@@ -83,38 +94,22 @@ struct PairRing {
   static constexpr int NS = DP + 2;        // rows i .. i+1+DP
   static constexpr int CS = 2 * DP + 2;    // class rows i .. i+1+2DP
   V N[NS][9][32];
-  V P[NS][32];
+  static constexpr int PS = DP + 3;        // phi rows i-1 .. i+1+DP
+  V P[PS][32];
   unsigned Cw[CS][32];
 };
 
-// collide the two nodes of a pair; fa/fb: node is fluid.  fp32: packed, masked; fp64: node by node
-__device__ __forceinline__ void collide_pair(const Consts<float>& C, const F2 (&n)[9], const F2 (&ph)[9],
-                                             bool fa, bool fb, F2 (&ns)[9], F2 (&bs)[9]) {
-  node_update_t<F2, float, true, true>(C, n, ph, ns, bs, nullptr, f2(fa ? 1.0f : 0.0f, fb ? 1.0f : 0.0f));
-  if (!(fa && fb)) {   // the solid partner stores zeros, so that its slots stay finite
+// collide the two nodes of a pair (fa/fb: node is fluid).  Both nodes always go through the
+// arithmetic together: packed FFMA2 in fp32, two interleaved dependency chains in fp64 (that is
+// what keeps the fp64 pipe busy at 2 warps per scheduler).  A node that is not fluid gets B* = 0
+// through the mask and stores N* = 0, so that its slots stay finite.
+template <typename R, typename V>
+__device__ __forceinline__ void collide_pair(const Consts<R>& C, const V (&n)[9], const V (&ph)[9],
+                                             bool fa, bool fb, V (&ns)[9], V (&bs)[9]) {
+  node_update_t<V, R, true, true>(C, n, ph, ns, bs, nullptr, mk(fa ? R(1) : R(0), fb ? R(1) : R(0)));
+  if (!(fa && fb)) {
 #pragma unroll
-    for (int q = 0; q < 9; q++) ns[q] = f2(fa ? ns[q].v.x : 0.0f, fb ? ns[q].v.y : 0.0f);
-  }
-}
-__device__ __forceinline__ void collide_pair(const Consts<double>& C, const D2 (&n)[9], const D2 (&ph)[9],
-                                             bool fa, bool fb, D2 (&ns)[9], D2 (&bs)[9]) {
-#pragma unroll
-  for (int q = 0; q < 9; q++) ns[q] = bs[q] = D2{0.0, 0.0};
-  if (fa) {
-    double n1[9], p1[9], s1[9], b1[9];
-#pragma unroll
-    for (int q = 0; q < 9; q++) { n1[q] = n[q].x; p1[q] = ph[q].x; }
-    node_update<double, true>(C, n1, p1, s1, b1, nullptr);
-#pragma unroll
-    for (int q = 0; q < 9; q++) { ns[q].x = s1[q]; bs[q].x = b1[q]; }
-  }
-  if (fb) {
-    double n1[9], p1[9], s1[9], b1[9];
-#pragma unroll
-    for (int q = 0; q < 9; q++) { n1[q] = n[q].y; p1[q] = ph[q].y; }
-    node_update<double, true>(C, n1, p1, s1, b1, nullptr);
-#pragma unroll
-    for (int q = 0; q < 9; q++) { ns[q].y = s1[q]; bs[q].y = b1[q]; }
+    for (int q = 0; q < 9; q++) ns[q] = mk(fa ? lo(ns[q]) : R(0), fb ? hi(ns[q]) : R(0));
   }
 }
 
@@ -127,7 +122,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   using V = typename PairOf<R>::type;
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int VB = 2 * (int)sizeof(R);   // bytes of a pair
-  constexpr int NS = Ring::NS, CS = Ring::CS;
+  constexpr int NS = Ring::NS, PS = Ring::PS, CS = Ring::CS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Ring& S = reinterpret_cast<Ring*>(smem_raw)[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
@@ -137,7 +132,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   constexpr unsigned N_STAGE = 9 * 32 * VB, N_PLANE = 32 * VB, P_STAGE = 32 * VB, C_STAGE = 32 * 4;
 
   const int nx = C.nx, ny = C.ny;   // nx is even (checked by the launcher)
-  const unsigned ps = (unsigned)C.ps;
+  const unsigned psB = (unsigned)C.ps * (unsigned)sizeof(R);   // plane stride in bytes (< 2^32: lbm_create)
   const int g = blockIdx.x * WARPS + (threadIdx.x >> 5);
   if (60 * g >= nx) return;                              // whole warp; the kernel has no block barrier
   const int xend = min(60 * g + 60, nx);                 // one past the last output column (even)
@@ -154,96 +149,88 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   const int rows = min(TY, ny - j0);
   const int last = rows + 1;                             // march row m = grid row j0-1+m; collided: 0..last
 
-  auto rowoff = [=](int m) -> unsigned {                 // element offset of march row m, periodic in y
+  auto wrap_row = [=](int m) -> int {                    // grid row of march row m, periodic in y
     int r = j0 - 1 + m;
-    r = r < 0 ? r + ny : (r >= ny ? r - ny : r);
-    return (unsigned)r * (unsigned)nx;
+    return r < 0 ? r + ny : (r >= ny ? r - ny : r);
   };
-  auto slotN = [](int m) { return (m + 1) % NS; };
-  auto slotC = [](int m) { return (m + 1) % CS; };
-  // ---- asynchronous fetches ----
-  auto issue_cls = [&](int m) {   // the two class words of the pair (one aligned 4-byte word)
-    cp_async_vec<4>(sC0 + (unsigned)slotC(m) * C_STAGE, cl16 + (rowoff(m) + (unsigned)xa));
+  auto inc = [](int v, int mod) { return v + 1 == mod ? 0 : v + 1; };
+  // ---- asynchronous fetches (slots and row offsets are passed in: no modulo in the march) ----
+  auto issue_cls = [&](unsigned u, int sc) {   // the two class words of the pair (one aligned 4-byte word)
+    cp_async_vec<4>(sC0 + (unsigned)sc * C_STAGE, cl16 + (u + (unsigned)xa));
   };
-  auto issue_row = [&](int m) {   // own-position populations and phi of march row m
-    const unsigned w2 = S.Cw[slotC(m)][lane];
+  // own-position populations and phi of one march row; lower/upper: the row feeds c_y <= 0 / c_y >= 0
+  auto issue_row = [&](unsigned u, int sn, int sp, int sc, bool lower, bool upper) {
+    const unsigned w2 = S.Cw[sc][lane];
     const unsigned ca = w2 & 0xffu, cb = (w2 >> 16) & 0xffu;
-    const unsigned k = rowoff(m) + (unsigned)xa;
-    const int sl = slotN(m);
-    if (ca != 3u || cb != 3u) cp_async_vec<VB>(sP0 + (unsigned)sl * P_STAGE, phi_in + k);
+    const unsigned k = u + (unsigned)xa;
+    if (ca != 3u || cb != 3u) cp_async_vec<VB>(sP0 + (unsigned)sp * P_STAGE, phi_in + k);
     if (ca < 2u || cb < 2u) {
-      const unsigned d = sN0 + (unsigned)sl * N_STAGE;
-      const bool lower = m >= 0, upper = m <= last;      // row -1 feeds only c_y = +1, row last+1 only c_y = -1
+      const unsigned d = sN0 + (unsigned)sn * N_STAGE;
+      const char* src = reinterpret_cast<const char*>(Nsrc + k);   // plane q is src + q * psB: one IMAD.WIDE each
       if (lower && upper) {
-        cp_async_vec<VB>(d + 0 * N_PLANE, Nsrc + k);
-        cp_async_vec<VB>(d + 1 * N_PLANE, Nsrc + (1u * ps + k));
-        cp_async_vec<VB>(d + 3 * N_PLANE, Nsrc + (3u * ps + k));
+        cp_async_vec<VB>(d + 0 * N_PLANE, src);
+        cp_async_vec<VB>(d + 1 * N_PLANE, src + (size_t)psB * 1u);
+        cp_async_vec<VB>(d + 3 * N_PLANE, src + (size_t)psB * 3u);
       }
       if (upper) {
-        cp_async_vec<VB>(d + 2 * N_PLANE, Nsrc + (2u * ps + k));
-        cp_async_vec<VB>(d + 5 * N_PLANE, Nsrc + (5u * ps + k));
-        cp_async_vec<VB>(d + 6 * N_PLANE, Nsrc + (6u * ps + k));
+        cp_async_vec<VB>(d + 2 * N_PLANE, src + (size_t)psB * 2u);
+        cp_async_vec<VB>(d + 5 * N_PLANE, src + (size_t)psB * 5u);
+        cp_async_vec<VB>(d + 6 * N_PLANE, src + (size_t)psB * 6u);
       }
       if (lower) {
-        cp_async_vec<VB>(d + 4 * N_PLANE, Nsrc + (4u * ps + k));
-        cp_async_vec<VB>(d + 7 * N_PLANE, Nsrc + (7u * ps + k));
-        cp_async_vec<VB>(d + 8 * N_PLANE, Nsrc + (8u * ps + k));
+        cp_async_vec<VB>(d + 4 * N_PLANE, src + (size_t)psB * 4u);
+        cp_async_vec<VB>(d + 7 * N_PLANE, src + (size_t)psB * 7u);
+        cp_async_vec<VB>(d + 8 * N_PLANE, src + (size_t)psB * 8u);
       }
     }
   };
 
-  // ---- prologue ----
+  // ---- prologue: ring slot of march row m is (m + 1) mod ring size ----
   {   // stale ring entries are read (and discarded) for solid nodes: they must be finite
     const V z = mk(R(0), R(0));
 #pragma unroll
-    for (int s = 0; s < NS; s++) {
+    for (int s = 0; s < NS; s++)
 #pragma unroll
       for (int q = 0; q < 9; q++) S.N[s][q][lane] = z;
-      S.P[s][lane] = z;
-    }
+#pragma unroll
+    for (int s = 0; s < PS; s++) S.P[s][lane] = z;
   }
   for (int m = -1; m <= 2 * DP; m++)
-    if (m <= last + 1) issue_cls(m);
+    if (m <= last + 1) issue_cls((unsigned)wrap_row(m) * (unsigned)nx, (m + 1) % CS);
   cp_async_commit();
   cp_async_wait<0>();
   for (int m = -1; m <= DP; m++) {
-    if (m <= last + 1) issue_row(m);
+    if (m <= last + 1)
+      issue_row((unsigned)wrap_row(m) * (unsigned)nx, (m + 1) % NS, (m + 1) % PS, (m + 1) % CS, m >= 0, m <= last);
     cp_async_commit();
   }
-  cp_async_wait<DP - 1>();   // rows -1, 0, 1 have landed
 
-  // carried between iterations (iteration i collides march row i)
-  V Bprev[3], Ccur[3];       // planes 2,5,6 of row i-1; planes 4,7,8 of row i
-  V phS[3], phC[3];          // phi of rows i-1 and i as (west, centre, east) vectors
-  {
-    const int sm1 = slotN(-1), s0 = slotN(0);
-    Bprev[0] = S.N[sm1][2][lane]; Bprev[1] = S.N[sm1][5][lane]; Bprev[2] = S.N[sm1][6][lane];
-    Ccur[0] = S.N[s0][4][lane]; Ccur[1] = S.N[s0][7][lane]; Ccur[2] = S.N[s0][8][lane];
-    const V a = S.P[sm1][lane], b = S.P[s0][lane];
-    phS[0] = from_left(a); phS[1] = a; phS[2] = from_right(a);
-    phC[0] = from_left(b); phC[1] = b; phC[2] = from_right(b);
-  }
+  // march state: ring slots of rows i-1, i, i+1 (populations, phi), of the rows being fetched, and
+  // the grid rows of the two fetch fronts
+  int sN_a = 0, sN_b = 1 % NS, sN_c = 2 % NS;
+  int sP_a = 0, sP_b = 1, sP_c = 2, sP_f = (DP + 2) % PS;
+  int sC_i = 1 % CS, sC_f = (DP + 2) % CS, sC_n = (2 * DP + 2) % CS;
+  int rf = wrap_row(DP + 1), rc = wrap_row(2 * DP + 1);
   unsigned kout = (unsigned)(j0 - 1) * (unsigned)nx + (unsigned)xa;   // own pair of march row i (1 <= i <= rows)
   const V zero = mk(R(0), R(0));
   V acc_prev = zero, up_prev = zero;
   bool fa_prev = false, fb_prev = false;
 
   for (int i = 0; i <= last; i++) {
-    if (i > 0) cp_async_wait<DP - 1>();   // row i+1 and the class words of row i+1+DP have landed
+    cp_async_wait<DP - 1>();   // row i+1 and the class words of row i+1+DP have landed
+    // operands that live in the slot about to be refilled: planes 2,5,6 of row i-1
+    const V Bp0 = S.N[sN_a][2][lane], Bp1 = S.N[sN_a][5][lane], Bp2 = S.N[sN_a][6][lane];
+    const V pS = S.P[sP_a][lane];
     // ---- issue: populations and phi of row i+1+DP, class words of row i+1+2DP ----
-    if (i + 1 + DP <= last + 1) issue_row(i + 1 + DP);
-    if (i + 1 + 2 * DP <= last + 1) issue_cls(i + 1 + 2 * DP);
+    if (i + 1 + DP <= last + 1) issue_row((unsigned)rf * (unsigned)nx, sN_a, sP_f, sC_f, true, i + 1 + DP <= last);
+    if (i + 1 + 2 * DP <= last + 1) issue_cls((unsigned)rc * (unsigned)nx, sC_n);
     cp_async_commit();
 
     // ---- on-chip operands of march row i ----
-    const int si = slotN(i), sn = slotN(i + 1);
-    const unsigned w2 = S.Cw[slotC(i)][lane];
-    const V A0 = S.N[si][0][lane], A1 = S.N[si][1][lane], A3 = S.N[si][3][lane];
-    V Bcur[3], Cnext[3];
-    Bcur[0] = S.N[si][2][lane]; Bcur[1] = S.N[si][5][lane]; Bcur[2] = S.N[si][6][lane];
-    Cnext[0] = S.N[sn][4][lane]; Cnext[1] = S.N[sn][7][lane]; Cnext[2] = S.N[sn][8][lane];
-    V phN[3];
-    phN[1] = S.P[sn][lane]; phN[0] = from_left(phN[1]); phN[2] = from_right(phN[1]);
+    const unsigned w2 = S.Cw[sC_i][lane];
+    const V A0 = S.N[sN_b][0][lane], A1 = S.N[sN_b][1][lane], A3 = S.N[sN_b][3][lane];
+    const V Cn0 = S.N[sN_c][4][lane], Cn1 = S.N[sN_c][7][lane], Cn2 = S.N[sN_c][8][lane];
+    const V pC = S.P[sP_b][lane], pN = S.P[sP_c][lane];
 
     const bool fa = (w2 & 0xffu) < 2u, fb = ((w2 >> 16) & 0xffu) < 2u;
     const unsigned lka = fa ? (w2 >> 8) & 0xffu : 0u, lkb = fb ? (w2 >> 24) : 0u;
@@ -251,11 +238,12 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
 
     // pulled populations: propagation A16-A17 on chip
     V nn[9];
-    nn[0] = A0;       nn[1] = from_left(A1);       nn[3] = from_right(A3);
-    nn[2] = Bprev[0]; nn[5] = from_left(Bprev[1]); nn[6] = from_right(Bprev[2]);
-    nn[4] = Cnext[0]; nn[7] = from_right(Cnext[1]); nn[8] = from_left(Cnext[2]);
+    nn[0] = A0;  nn[1] = from_left(A1);   nn[3] = from_right(A3);
+    nn[2] = Bp0; nn[5] = from_left(Bp1);  nn[6] = from_right(Bp2);
+    nn[4] = Cn0; nn[7] = from_right(Cn1); nn[8] = from_left(Cn2);
     if (any_link) {   // warp-uniform; half-way bounce-back (R12): own opposite population, same row
-      const V own[9] = {A0, A1, Bcur[0], A3, Ccur[0], Bcur[1], Bcur[2], Ccur[1], Ccur[2]};   // plane q at (x, i)
+      const V own[9] = {A0, A1, S.N[sN_b][2][lane], A3, S.N[sN_b][4][lane], S.N[sN_b][5][lane],
+                        S.N[sN_b][6][lane], S.N[sN_b][7][lane], S.N[sN_b][8][lane]};   // plane q at (x, i)
 #pragma unroll
       for (int q = 1; q < 9; q++) {
         const V o = own[opp(q)];
@@ -265,12 +253,29 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
         nn[q] = mk(a, b);
       }
     }
+    const unsigned fmask = __ballot_sync(FULL, col_out && (fa || fb));
+    const bool st = col_out && i >= 1 && i <= rows && (fmask & gmask) != 0u;   // my sector holds a fluid node
 
-    V ns[9], bs[9];
+    // phi stencil (R8): west / east neighbours of the three rows (shuffles: all lanes take part)
+    const V pCw = from_left(pC), pCe = from_right(pC), pNw = from_left(pN), pNe = from_right(pN);
+    const V pSw = from_left(pS), pSe = from_right(pS);
+
+    V bs[9];
     V bb = zero;
-    if (fa || fb) {
-      const V ph[9] = {phC[1], phC[2], phN[1], phC[0], phS[1], phN[2], phN[0], phS[0], phS[2]};
-      collide_pair(C, nn, ph, fa, fb, ns, bs);
+    if (fa || fb || st) {   // st without a fluid node: a solid pair completing a sector with zeros
+      const V ph[9] = {pC, pCe, pN, pCw, pS, pNe, pNw, pSw, pSe};
+      V ns[9];
+      collide_pair<R, V>(C, nn, ph, fa, fb, ns, bs);
+      if (st) {
+        char* dst = reinterpret_cast<char*>(Ndst + kout);
+#pragma unroll
+        for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dst + (size_t)psB * (unsigned)q) = ns[q];
+        if (WRITE_B) {
+          char* dstB = reinterpret_cast<char*>(Bdst + kout);
+#pragma unroll
+          for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dstB + (size_t)psB * (unsigned)q) = bs[q];
+        }
+      }
       if (lka | lkb) {   // link q hands the node its own B_opp(q)* back
         R ba = R(0), bbv = R(0);
 #pragma unroll
@@ -282,19 +287,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       }
     } else {
 #pragma unroll
-      for (int q = 0; q < 9; q++) ns[q] = bs[q] = zero;
-    }
-    {
-      const bool row_out = i >= 1 && i <= rows;
-      const unsigned fmask = __ballot_sync(FULL, col_out && (fa || fb));
-      if (row_out && col_out && (fmask & gmask) != 0u) {
-#pragma unroll
-        for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(Ndst + ((unsigned)q * ps + kout)) = ns[q];
-        if (WRITE_B) {
-#pragma unroll
-          for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(Bdst + ((unsigned)q * ps + kout)) = bs[q];
-        }
-      }
+      for (int q = 0; q < 9; q++) bs[q] = zero;
     }
     // contributions of row i to phi(t+1) of rows i-1 (down), i (mid), i+1 (up)
     const V mid = bs[0] + from_left(bs[1]) + from_right(bs[3]);
@@ -314,8 +307,10 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     fa_prev = fa; fb_prev = fb;
 
     kout += (unsigned)nx;
-#pragma unroll
-    for (int t = 0; t < 3; t++) { Bprev[t] = Bcur[t]; Ccur[t] = Cnext[t]; phS[t] = phC[t]; phC[t] = phN[t]; }
+    sN_a = sN_b; sN_b = sN_c; sN_c = inc(sN_c, NS);
+    sP_a = sP_b; sP_b = sP_c; sP_c = inc(sP_c, PS); sP_f = inc(sP_f, PS);
+    sC_i = inc(sC_i, CS); sC_f = inc(sC_f, CS); sC_n = inc(sC_n, CS);
+    rf = inc(rf, ny); rc = inc(rc, ny);
   }
   cp_async_wait<0>();
 }
