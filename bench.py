@@ -120,12 +120,28 @@ def cpu_oracle_rate(steps: int, warmup: int, budget_s: float = 25.0):
                 mflups=w.meta["n_fluid"] * steps / dt / 1e6, ms_per_step=dt / steps * 1e3, steps=steps, n=n)
 
 
+def max_over_ranks(values, dist, device):
+    """Multi-GPU timing rule: every reported time is the MAX over ranks (replicas only: there is no
+    data-path collective; torch.distributed carries just this reduction and the barriers)."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def replica_seed(rank: int) -> int:
+    """Replicas: the same recipe with a rank-specific seed."""
+    return int(rank)
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     steps = max(1, args.steps)
-    cb = cpu_oracle_rate(steps, max(0, min(args.warmup, 3)), budget_s=120.0)
+    cb = cpu_oracle_rate(steps, max(0, min(args.warmup, 3)), budget_s=args.reference_budget)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": "MLUPS", "n_gpus": args.gpus,
             "steps": cb["steps"], "warmup": min(args.warmup, 3), "ms_per_step": cb["ms_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -195,10 +211,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
     t_e2e = time.perf_counter() - t0
     dg = sim.diag()
 
-    if dist is not None:
-        tt = torch.tensor([ms, t_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms, t_e2e = float(tt[0]), float(tt[1])
+    ms, t_e2e = max_over_ranks([ms, t_e2e], dist, "cuda")
 
     fused = schedule != binding.SCHEDULE_BASELINE
     values = 20 if fused else 38
@@ -236,6 +249,7 @@ def main():
     ap.add_argument("--precision", default="both", choices=["64", "32", "both"])
     ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "warp", "pair"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--reference-budget", type=float, default=120.0, help="seconds of CPU work the --impl reference arm may spend")
     ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"),
                     help="ncu dram bytes per launch of the dominant kernel, written by hand from an ncu capture")
     args = ap.parse_args()
@@ -262,7 +276,7 @@ def main():
 
     sched = {"auto": binding.SCHEDULE_AUTO, "baseline": binding.SCHEDULE_BASELINE, "fused": binding.SCHEDULE_FUSED,
              "warp": binding.SCHEDULE_WARP, "pair": binding.SCHEDULE_PAIR}[args.schedule]
-    w = wl.config5(seed=rank, n=args.n)                # replicas: same recipe, rank-specific seed
+    w = wl.config5(seed=replica_seed(rank), n=args.n)   # replicas: same recipe, rank-specific seed
     precs = [64, 32] if args.precision == "both" else [int(args.precision)]
     results = {p: bench_precision(args, w, p, sched, local, dist) for p in precs}
 

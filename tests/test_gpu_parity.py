@@ -295,3 +295,45 @@ def test_schedules_agree_and_get_is_idempotent(sched):
         b.get_populations(want_B=True)                 # B is not stored unless keep_B was set
     lc = b.launch_counts()
     assert lc["collide"] == 25 and lc["phi_sum"] == 0 and lc["ghost"] == 26
+
+
+# ---- throughput workload (config 5) in the launch configuration bench.py times ---------------------
+@pytest.mark.parametrize("precision", [64, 32])
+def test_config5_2048_against_oracle(precision):
+    """Porous medium at 2048^2 (first size of BASELINE config 5; same recipe, launch schedule and
+    kernel as bench.py's 8192^2): full fields against the oracle after a few steps."""
+    w = wl.config5(seed=1, n=2048)
+    g, o = make_pair(w, precision=precision)               # schedule AUTO = what bench.py runs
+    g.init(w.phi0); o.init(w.phi0)
+    g.step(3); o.step(3)
+    err, scale = field_errors(g, o)
+    uscale = max(scale["ux"], scale["uy"], w.sigma / (w.rho_l * w.nu_l))
+    print("config5 2048", precision, err, scale)
+    tol = 1e-12 if precision == 64 else 2e-4
+    assert err["phi"] <= tol
+    assert max(err["ux"], err["uy"]) <= (tol if precision == 64 else tol * uscale)
+    assert err["rho"] <= tol * scale["rho"]
+
+
+def test_config5_8192_properties_and_samples():
+    """bench.py's exact workload (8192^2, seed 0, schedule AUTO).  The oracle needs minutes per step
+    at this size, so: (i) per-phase mass is conserved (sum B_i* = phi), (ii) no NaN,
+    phi stays in range, (iii) sampled nodes agree with the BASELINE schedule (independent kernels,
+    N and B both in HBM), which the smaller tests pin to the oracle."""
+    w = wl.config5(seed=0, n=8192)
+    rng = np.random.default_rng(5)
+    fl = np.flatnonzero(w.mask.reshape(-1) == 0)
+    idx = np.sort(rng.choice(fl, 200000, replace=False)).astype(np.int64)
+    from paper_2605_30878_b200 import binding
+    res = {}
+    for sched in (0, BASELINE):
+        s = binding.LBM(binding.LBMParams(precision=64, schedule=sched, **w.param_dict()), w.mask, w.disks)
+        s.init(w.phi0)
+        d0 = s.diag()
+        s.step(20)
+        d1 = s.diag()
+        assert d1["nan"] == 0 and -1e-3 < d1["phi_min"] and d1["phi_max"] < 1 + 1e-3
+        assert abs(d1["sum_phi"] - d0["sum_phi"]) <= 1e-11 * d0["sum_phi"]
+        res[sched] = s.sample_populations(idx)[0]
+        s.close()
+    assert np.abs(res[0] - res[BASELINE]).max() <= 1e-13
