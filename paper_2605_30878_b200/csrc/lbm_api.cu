@@ -1,6 +1,7 @@
 // lbm_api.cu — host side of liblbm_b200.so: the C ABI of include/lbm.h, workspace carving and
 // the launch schedule.  No CPU fallback: every compute call needs a CUDA device.
 #include <cuda_runtime.h>
+#include <cub/device/device_radix_sort.cuh>
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -58,6 +59,11 @@ struct lbm_ctx {
   double* wgt_d;
   double *gnx, *gny, *gdepth;
   uint8_t* csolid;
+  // the same list in the ghost kernel's processing order (tile-major)
+  int* gidx_p;
+  int* corner_p;
+  void* wgt_p;
+  uint8_t* csolid_p;
   int* blk_cnt;
   int* blk_off;
   int* scal;          // [0] ghost total, [1] geometry error flag
@@ -162,10 +168,15 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
   double* gny = A.take<double>(g);
   double* gdepth = A.take<double>(g);
   uint8_t* csolid = A.take<uint8_t>(g);
+  int* gidx_p = A.take<int>(g);
+  int* corner_p = A.take<int>(4 * g);
+  char* wgt_p = A.take<char>(4 * g * rs);
+  uint8_t* csolid_p = A.take<uint8_t>(g);
   if (c && base) {
     c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
     c->cls = cls; c->links = links; c->cl16 = cl16; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
-    c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid; c->blk_cnt = blk_cnt;
+    c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid;
+    c->gidx_p = gidx_p; c->corner_p = corner_p; c->wgt_p = wgt_p; c->csolid_p = csolid_p; c->blk_cnt = blk_cnt;
     c->blk_off = blk_off; c->scal = scal; c->stage = stage; c->diag_out = diag_out;
     c->samp_idx = samp; c->samp_cap = samp_cap;
   }
@@ -208,7 +219,7 @@ template <typename R>
 void launch_ghost(lbm_ctx* c) {
   if (c->ng == 0) return;
   k_ghost_update<R><<<(c->ng + 127) / 128, 128, 0, c->st>>>(
-      consts_of<R>(c), c->ng, c->gidx, (const int4*)c->corner, (const R*)c->wgt, c->csolid,
+      consts_of<R>(c), c->ng, c->gidx_p, (const int4*)c->corner_p, (const R*)c->wgt_p, c->csolid_p,
       (const R*)c->phi[c->pcur ^ 1], (R*)c->phi[c->pcur]);
   c->launches[2]++;
 }
@@ -393,6 +404,33 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     if (bad) {
       delete c;
       return fail(nullptr, LBM_EINVAL, "mask and geometry disagree: a ghost node lies in no disk");
+    }
+    // tile-major processing order for the ghost update (one-time; temporaries are freed again)
+    {
+      unsigned *k_in = nullptr, *k_out = nullptr;
+      int *v_in = nullptr, *v_out = nullptr;
+      void* tmp = nullptr;
+      size_t tmp_bytes = 0;
+      cudaError_t e = cudaMalloc(&k_in, 4 * sizeof(int) * (size_t)ng);
+      if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(ghost order)"); }
+      k_out = k_in + ng; v_in = reinterpret_cast<int*>(k_out + ng); v_out = v_in + ng;
+      k_ghost_tile_keys<<<(ng + 255) / 256, 256, 0, c->st>>>(ng, c->gidx, prm->nx, k_in, v_in);
+      e = cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, k_in, k_out, v_in, v_out, ng, 0, 32, c->st);
+      if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 1);
+      if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k_in, k_out, v_in, v_out, ng, 0, 32, c->st);
+      if (e == cudaSuccess) {
+        if (c->is32)
+          k_ghost_permute<float><<<(ng + 255) / 256, 256, 0, c->st>>>(ng, v_out, c->gidx, (const int4*)c->corner, (const float*)c->wgt,
+                                                                      c->csolid, c->gidx_p, (int4*)c->corner_p, (float*)c->wgt_p, c->csolid_p);
+        else
+          k_ghost_permute<double><<<(ng + 255) / 256, 256, 0, c->st>>>(ng, v_out, c->gidx, (const int4*)c->corner, (const double*)c->wgt,
+                                                                       c->csolid, c->gidx_p, (int4*)c->corner_p, (double*)c->wgt_p, c->csolid_p);
+        e = cudaGetLastError();
+      }
+      if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+      cudaFree(tmp);
+      cudaFree(k_in);
+      if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "ghost processing order"); }
     }
   }
   CKC(cudaStreamSynchronize(c->st));

@@ -218,6 +218,35 @@ __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __res
   csolid[g] = (uint8_t)((cls[c0] >= 2) | ((cls[c1] >= 2) << 1) | ((cls[c2] >= 2) << 2) | ((cls[c3] >= 2) << 3));
 }
 
+// Processing order of the ghost update: tile-major (32 x 32 node tiles, index order inside a tile),
+// so that the ghosts of one CTA gather phi from the same few sectors (L1 hits instead of DRAM
+// re-fetches; the index-sorted list, the API's order, strides over the whole row between
+// neighbours).  The update is a Jacobi sweep (R13): the order does not change any value.
+__global__ void __launch_bounds__(256) k_ghost_tile_keys(int ng, const int* __restrict__ gidx, int nx,
+                                                         unsigned* __restrict__ keys, int* __restrict__ vals) {
+  const int g = blockIdx.x * 256 + threadIdx.x;
+  if (g >= ng) return;
+  const int k = gidx[g];
+  const int i = k % nx, j = k / nx;
+  keys[g] = (unsigned)(j >> 5) * (unsigned)((nx + 31) >> 5) + (unsigned)(i >> 5);
+  vals[g] = g;
+}
+template <typename R>
+__global__ void __launch_bounds__(256) k_ghost_permute(int ng, const int* __restrict__ perm,
+                                                       const int* __restrict__ gidx, const int4* __restrict__ corner,
+                                                       const R* __restrict__ wgt, const uint8_t* __restrict__ csolid,
+                                                       int* __restrict__ gidx_p, int4* __restrict__ corner_p,
+                                                       R* __restrict__ wgt_p, uint8_t* __restrict__ csolid_p) {
+  const int t = blockIdx.x * 256 + threadIdx.x;
+  if (t >= ng) return;
+  const int g = perm[t];
+  gidx_p[t] = gidx[g];
+  corner_p[t] = corner[g];
+#pragma unroll
+  for (int c = 0; c < 4; c++) wgt_p[4 * t + c] = wgt[4 * g + c];
+  csolid_p[t] = csolid[g];
+}
+
 // ------------------------------------------------------------------------------------------
 // (2) ghost-node order-parameter update, Eq. 9 (:78-80): phi_F by bilinear interpolation at
 // x_F = x_G + n_s (:66); Jacobi (R13): fluid corners carry this time's phi (phi_cur), solid
