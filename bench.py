@@ -215,7 +215,8 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
 
     fused = schedule != binding.SCHEDULE_BASELINE
     values = 20 if fused else 38
-    bytes_layout = n_fluid * values * rs + n          # + 1 class byte per node
+    cls_bytes = 2 if schedule in (binding.SCHEDULE_AUTO, binding.SCHEDULE_PAIR, binding.SCHEDULE_WARP) else 1
+    bytes_layout = n_fluid * values * rs + cls_bytes * n   # + the class word of every node (cl16: 2 B)
     bytes_canon = n_fluid * (36 * rs + 1)
     peak, peak_src = measured_peak()
     ach = bytes_layout / t_collide / 1e9
@@ -250,8 +251,9 @@ def main():
     ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "warp", "pair"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--reference-budget", type=float, default=120.0, help="seconds of CPU work the --impl reference arm may spend")
-    ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"),
-                    help="ncu dram bytes per launch of the dominant kernel, written by hand from an ncu capture")
+    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r1_traffic.csv"),
+                    help="ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel "
+                         "(kernel,precision,n,dram_bytes_read,dram_bytes_write), copied from an ncu --set full capture")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -288,15 +290,19 @@ def main():
     if rank == 0:
         main_p = precs[0]
         r = results[main_p]
-        traffic = None
-        try:
-            with open(args.traffic_json) as f:
-                tj = json.load(f)
-            key = f"{r['roofline']['kernel']}_f{main_p}_n{args.n}"
-            traffic = tj.get(key, {}).get("dram_bytes_per_launch")
-        except Exception:
-            pass
-        r["roofline"]["traffic"] = traffic
+        def lookup_traffic(kernel, prec):
+            try:
+                with open(args.traffic_csv) as f:
+                    for ln in f:
+                        c = [x.strip() for x in ln.split(",")]
+                        if len(c) >= 5 and c[0] == kernel and c[1] == str(prec) and c[2] == str(args.n):
+                            return float(c[3]) + float(c[4])
+            except Exception:
+                pass
+            return None
+
+        for p_, q_ in results.items():
+            q_["roofline"]["traffic"] = lookup_traffic(q_["roofline"]["kernel"], p_)
         line = {
             "metric": METRIC, "value": r["mlups"] * world, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": r["ms"] / args.steps, "higher_is_better": True, "scaling": "weak",

@@ -253,7 +253,7 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     const R* pi = (const R*)c->phi[c->pcur];
     R* po = (R*)c->phi[c->pcur ^ 1];
     bool done = false;
-    if (c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair<R>(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
+    if (c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
     if (!done && c->sched == LBM_SCHEDULE_WARP) done = launch_fused_warp<R>(C, c->cl16, Ns, Nd, Bd, pi, po, c->st) == 0;
     if (!done) launch_fused_step<R>(C, c->cls, c->links, Ns, Nd, Bd, pi, po, c->st);
     c->cur ^= 1;

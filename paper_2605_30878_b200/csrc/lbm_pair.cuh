@@ -1,19 +1,23 @@
 // lbm_pair.cuh — PAIR schedule: the fused pull-stream + collide + segregation + phi(t+1) kernel in
-// which every lane owns TWO x-adjacent nodes (an aligned pair), every value moves as an aligned
-// 8-byte (fp32) or 16-byte (fp64) vector, and fp32 arithmetic is packed (FFMA2/FADD2/FMUL2).
-// Same arithmetic per node as the other schedules (node_update_t), same HBM state.
+// which every lane owns NL x-adjacent nodes (an aligned group: 2 in fp64, 4 in fp32, 2 in fp32 when
+// nx is not a multiple of 4), every value moves as an aligned 8- or 16-byte vector, and fp32
+// arithmetic is packed (FFMA2/FADD2/FMUL2).  Same arithmetic per node as the other schedules
+// (node_update_t), same HBM state.
 //
-//   * a warp owns a strip of 64 columns [60 g - 2, 60 g + 62): 60 output columns and two halo
-//     columns per side (one is needed; pairs must stay aligned), and marches down TY rows (+1 halo
-//     row per end).  No shared data between warps, no block barrier.
+//   * a warp owns a strip of 32 NL columns: 30 NL output columns and one halo LANE per side (only
+//     the halo column next to the outputs is needed; groups must stay aligned), and marches down TY
+//     rows (+1 halo row per end).  No shared data between warps, no block barrier.
 //   * every population is fetched from HBM exactly once per strip, UNSHIFTED, at its own node, by
-//     cp.async (LDGSTS) into a private shared-memory ring DP+1 rows ahead of the collision; pairs
+//     cp.async (LDGSTS) into a private shared-memory ring DP+1 rows ahead of the collision; groups
 //     with no fluid node are not fetched.  Propagation (A16-A17, :318-322) is done on chip: the row
 //     part by reading the ring slot of the neighbouring row, the column part by one warp shuffle
 //     per shifted plane.  Half-way bounce-back (R12) selects the node's own opposite population,
 //     which is already on chip.
-//   * phi(x, t+1) = sum_q B_q*(x - c_q, t) (A13) is assembled in registers as in lbm_warp.cuh.
-//   * stores are aligned vectors at the node's own position.
+//   * phi(x, t+1) = sum_q B_q*(x - c_q, t) (A13) is assembled in registers: the B* that move in x
+//     shift through the lane's registers and one shuffle, the row moves are carried from one march
+//     row to the next; links add the node's own B_opp(q)*.
+//   * stores are aligned vectors at the node's own position; a 32-byte sector that holds any fluid
+//     node is written whole (zeros on its solid nodes): partial sectors made HBM read-modify-write.
 #pragma once
 #include "lbm_kernels.cuh"
 #include "lbm_warp.cuh"   // cp_async_commit / cp_async_wait
@@ -33,6 +37,9 @@ namespace lbm {
 #ifndef LBM_PAIR_MINB64
 #define LBM_PAIR_MINB64 3
 #endif
+#ifndef LBM_PAIR_MINBQ
+#define LBM_PAIR_MINBQ 3
+#endif
 #ifndef LBM_PAIR_WARPS
 #define LBM_PAIR_WARPS 4
 #endif
@@ -42,21 +49,18 @@ namespace lbm {
 #ifndef LBM_PAIR_TY
 #define LBM_PAIR_TY 64
 #endif
+#ifndef LBM_PAIR_QUAD
+#define LBM_PAIR_QUAD 0   // 4 nodes per lane in fp32: measured equal to 2 (0.96 vs 0.97 ms), kept as a build knob
+#endif
 
-// ---- pair value types ----
-struct __align__(16) D2 {   // two fp64 nodes; arithmetic is done node by node (no packed fp64 instructions)
+// ---- lane value types: NL nodes of one lane ----
+struct __align__(16) D2 {   // two fp64 nodes: two interleaved dependency chains
   double x, y;
 };
-template <typename R> struct PairOf;
-template <> struct PairOf<float> { using type = F2; };
-template <> struct PairOf<double> { using type = D2; };
+struct __align__(16) Q4 {   // four fp32 nodes: two packed f32x2 streams
+  F2 a, b;
+};
 
-__device__ __forceinline__ float lo(F2 a) { return a.v.x; }
-__device__ __forceinline__ float hi(F2 a) { return a.v.y; }
-__device__ __forceinline__ double lo(D2 a) { return a.x; }
-__device__ __forceinline__ double hi(D2 a) { return a.y; }
-__device__ __forceinline__ F2 mk(float a, float b) { return f2(a, b); }
-__device__ __forceinline__ D2 mk(double a, double b) { return D2{a, b}; }
 __device__ __forceinline__ D2 operator+(D2 a, D2 b) { return D2{a.x + b.x, a.y + b.y}; }
 __device__ __forceinline__ D2 operator-(D2 a, D2 b) { return D2{a.x - b.x, a.y - b.y}; }
 __device__ __forceinline__ D2 operator*(D2 a, D2 b) { return D2{a.x * b.x, a.y * b.y}; }
@@ -70,14 +74,71 @@ __device__ __forceinline__ D2 operator*(double a, D2 b) { return D2{a * b.x, a *
 __device__ __forceinline__ D2 rcp_(D2 a) { return D2{1.0 / a.x, 1.0 / a.y}; }
 __device__ __forceinline__ D2 rsqrt0_(D2 a) { return D2{rsqrt0_(a.x), rsqrt0_(a.y)}; }
 
-// propagation in x: value arriving from the left neighbour (c_x = +1) / right neighbour (c_x = -1)
+__device__ __forceinline__ Q4 operator+(Q4 a, Q4 b) { return Q4{a.a + b.a, a.b + b.b}; }
+__device__ __forceinline__ Q4 operator-(Q4 a, Q4 b) { return Q4{a.a - b.a, a.b - b.b}; }
+__device__ __forceinline__ Q4 operator*(Q4 a, Q4 b) { return Q4{a.a * b.a, a.b * b.b}; }
+__device__ __forceinline__ Q4 operator-(Q4 a) { return Q4{-a.a, -a.b}; }
+__device__ __forceinline__ Q4 operator+(Q4 a, float b) { return Q4{a.a + b, a.b + b}; }
+__device__ __forceinline__ Q4 operator+(float a, Q4 b) { return Q4{a + b.a, a + b.b}; }
+__device__ __forceinline__ Q4 operator-(Q4 a, float b) { return Q4{a.a - b, a.b - b}; }
+__device__ __forceinline__ Q4 operator-(float a, Q4 b) { return Q4{a - b.a, a - b.b}; }
+__device__ __forceinline__ Q4 operator*(Q4 a, float b) { return Q4{a.a * b, a.b * b}; }
+__device__ __forceinline__ Q4 operator*(float a, Q4 b) { return Q4{a * b.a, a * b.b}; }
+__device__ __forceinline__ Q4 rcp_(Q4 a) { return Q4{rcp_(a.a), rcp_(a.b)}; }
+__device__ __forceinline__ Q4 rsqrt0_(Q4 a) { return Q4{rsqrt0_(a.a), rsqrt0_(a.b)}; }
+
+// traits: scalar type, nodes per lane, (un)packing into per-node scalars
+template <typename V> struct LaneOf;
+template <> struct LaneOf<F2> {
+  using R = float;
+  static constexpr int NL = 2;
+  static __device__ __forceinline__ void unpack(F2 v, float (&x)[2]) { x[0] = v.v.x; x[1] = v.v.y; }
+  static __device__ __forceinline__ F2 pack(const float (&x)[2]) { return f2(x[0], x[1]); }
+};
+template <> struct LaneOf<D2> {
+  using R = double;
+  static constexpr int NL = 2;
+  static __device__ __forceinline__ void unpack(D2 v, double (&x)[2]) { x[0] = v.x; x[1] = v.y; }
+  static __device__ __forceinline__ D2 pack(const double (&x)[2]) { return D2{x[0], x[1]}; }
+};
+template <> struct LaneOf<Q4> {
+  using R = float;
+  static constexpr int NL = 4;
+  static __device__ __forceinline__ void unpack(Q4 v, float (&x)[4]) {
+    x[0] = v.a.v.x; x[1] = v.a.v.y; x[2] = v.b.v.x; x[3] = v.b.v.y;
+  }
+  static __device__ __forceinline__ Q4 pack(const float (&x)[4]) { return Q4{f2(x[0], x[1]), f2(x[2], x[3])}; }
+};
+
+// propagation in x by one node: the value arriving from the left neighbour (c_x = +1) / from the
+// right neighbour (c_x = -1); one element crosses the lane boundary by shuffle
 template <typename V>
 __device__ __forceinline__ V from_left(V a) {
-  return mk(__shfl_up_sync(0xffffffffu, hi(a), 1), lo(a));
+  using L = LaneOf<V>;
+  typename L::R x[L::NL], y[L::NL];
+  L::unpack(a, x);
+  y[0] = __shfl_up_sync(0xffffffffu, x[L::NL - 1], 1);
+#pragma unroll
+  for (int c = 1; c < L::NL; c++) y[c] = x[c - 1];
+  return L::pack(y);
 }
 template <typename V>
 __device__ __forceinline__ V from_right(V a) {
-  return mk(hi(a), __shfl_down_sync(0xffffffffu, lo(a), 1));
+  using L = LaneOf<V>;
+  typename L::R x[L::NL], y[L::NL];
+  L::unpack(a, x);
+#pragma unroll
+  for (int c = 0; c < L::NL - 1; c++) y[c] = x[c + 1];
+  y[L::NL - 1] = __shfl_down_sync(0xffffffffu, x[0], 1);
+  return L::pack(y);
+}
+template <typename V>
+__device__ __forceinline__ V splat(typename LaneOf<V>::R s) {
+  using L = LaneOf<V>;
+  typename L::R x[L::NL];
+#pragma unroll
+  for (int c = 0; c < L::NL; c++) x[c] = s;
+  return L::pack(x);
 }
 
 template <int BYTES>
@@ -86,64 +147,79 @@ __device__ __forceinline__ void cp_async_vec(unsigned saddr, const void* gptr) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(saddr), "l"(gptr), "n"(BYTES) : "memory");
 }
 
-// shared-memory ring of one warp: row stages hold the own-position populations and phi of the 64
-// columns; class stages the packed class words (two 16-bit words per lane)
-template <typename R, int DP>
+// shared-memory ring of one warp: row stages hold the own-position populations and phi of the strip;
+// class stages the packed class words (NL 16-bit words per lane)
+template <typename V, int DP>
 struct PairRing {
-  using V = typename PairOf<R>::type;
-  static constexpr int NS = DP + 2;        // rows i .. i+1+DP
+  static constexpr int NL = LaneOf<V>::NL;
+  static constexpr int NS = DP + 2;        // population rows i-1 (until refilled) .. i+1+DP
+  static constexpr int PS = DP + 3;        // phi rows i-1 .. i+1+DP
   static constexpr int CS = 2 * DP + 2;    // class rows i .. i+1+2DP
   V N[NS][9][32];
-  static constexpr int PS = DP + 3;        // phi rows i-1 .. i+1+DP
   V P[PS][32];
-  unsigned Cw[CS][32];
+  unsigned short Cw[CS][32][NL];
 };
 
-// collide the two nodes of a pair (fa/fb: node is fluid).  Both nodes always go through the
-// arithmetic together: packed FFMA2 in fp32, two interleaved dependency chains in fp64 (that is
-// what keeps the fp64 pipe busy at 2 warps per scheduler).  A node that is not fluid gets B* = 0
-// through the mask and stores N* = 0, so that its slots stay finite.
-template <typename R, typename V>
-__device__ __forceinline__ void collide_pair(const Consts<R>& C, const V (&n)[9], const V (&ph)[9],
-                                             bool fa, bool fb, V (&ns)[9], V (&bs)[9]) {
-  node_update_t<V, R, true, true>(C, n, ph, ns, bs, nullptr, mk(fa ? R(1) : R(0), fb ? R(1) : R(0)));
-  if (!(fa && fb)) {
+// collide the NL nodes of a lane (fl[c]: node c is fluid).  All nodes always go through the
+// arithmetic together: packed FFMA2 in fp32, interleaved dependency chains in fp64.  A node that is
+// not fluid gets B* = 0 through the mask and stores N* = 0, so that its slots stay finite.
+template <typename V>
+__device__ __forceinline__ void collide_lane(const Consts<typename LaneOf<V>::R>& C, const V (&n)[9],
+                                             const V (&ph)[9], const bool (&fl)[LaneOf<V>::NL], bool all_fluid,
+                                             V (&ns)[9], V (&bs)[9]) {
+  using L = LaneOf<V>;
+  using R = typename L::R;
+  R m[L::NL];
 #pragma unroll
-    for (int q = 0; q < 9; q++) ns[q] = mk(fa ? lo(ns[q]) : R(0), fb ? hi(ns[q]) : R(0));
+  for (int c = 0; c < L::NL; c++) m[c] = fl[c] ? R(1) : R(0);
+  node_update_t<V, R, true, true>(C, n, ph, ns, bs, nullptr, L::pack(m));
+  if (!all_fluid) {
+#pragma unroll
+    for (int q = 0; q < 9; q++) {
+      R x[L::NL];
+      L::unpack(ns[q], x);
+#pragma unroll
+      for (int c = 0; c < L::NL; c++) x[c] = fl[c] ? x[c] : R(0);
+      ns[q] = L::pack(x);
+    }
   }
 }
 
-template <typename R, int DP, int WARPS, int MINB, bool WRITE_B>
+template <typename V, int DP, int WARPS, int MINB, bool WRITE_B>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
-    k_fused_pair(const Consts<R> C, const uint16_t* __restrict__ cl16, const R* __restrict__ Nsrc,
-                 R* __restrict__ Ndst, R* __restrict__ Bdst, const R* __restrict__ phi_in,
-                 R* __restrict__ phi_out, int TY) {
-  using Ring = PairRing<R, DP>;
-  using V = typename PairOf<R>::type;
+    k_fused_pair(const Consts<typename LaneOf<V>::R> C, const uint16_t* __restrict__ cl16,
+                 const typename LaneOf<V>::R* __restrict__ Nsrc, typename LaneOf<V>::R* __restrict__ Ndst,
+                 typename LaneOf<V>::R* __restrict__ Bdst, const typename LaneOf<V>::R* __restrict__ phi_in,
+                 typename LaneOf<V>::R* __restrict__ phi_out, int TY) {
+  using L = LaneOf<V>;
+  using R = typename L::R;
+  using Ring = PairRing<V, DP>;
+  constexpr int NL = L::NL;
+  constexpr int OUTC = 30 * NL;            // output columns of a strip
   constexpr unsigned FULL = 0xffffffffu;
-  constexpr int VB = 2 * (int)sizeof(R);   // bytes of a pair
+  constexpr int VB = NL * (int)sizeof(R);  // bytes of a lane vector
   constexpr int NS = Ring::NS, PS = Ring::PS, CS = Ring::CS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Ring& S = reinterpret_cast<Ring*>(smem_raw)[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
   const unsigned sN0 = (unsigned)__cvta_generic_to_shared(&S.N[0][0][lane]);
   const unsigned sP0 = (unsigned)__cvta_generic_to_shared(&S.P[0][lane]);
-  const unsigned sC0 = (unsigned)__cvta_generic_to_shared(&S.Cw[0][lane]);
-  constexpr unsigned N_STAGE = 9 * 32 * VB, N_PLANE = 32 * VB, P_STAGE = 32 * VB, C_STAGE = 32 * 4;
+  const unsigned sC0 = (unsigned)__cvta_generic_to_shared(&S.Cw[0][lane][0]);
+  constexpr unsigned N_STAGE = 9 * 32 * VB, N_PLANE = 32 * VB, P_STAGE = 32 * VB, C_STAGE = 32 * NL * 2;
 
-  const int nx = C.nx, ny = C.ny;   // nx is even (checked by the launcher)
+  const int nx = C.nx, ny = C.ny;   // nx is a multiple of NL (checked by the launcher)
   const unsigned psB = (unsigned)C.ps * (unsigned)sizeof(R);   // plane stride in bytes (< 2^32: lbm_create)
   const int g = blockIdx.x * WARPS + (threadIdx.x >> 5);
-  if (60 * g >= nx) return;                              // whole warp; the kernel has no block barrier
-  const int xend = min(60 * g + 60, nx);                 // one past the last output column (even)
-  const int lxa = 60 * g - 2 + 2 * lane;                 // logical column of the pair's first node
+  if (OUTC * g >= nx) return;                            // whole warp; the kernel has no block barrier
+  const int xend = min(OUTC * g + OUTC, nx);             // one past the last output column (multiple of NL)
+  const int lxa = OUTC * g - NL + NL * lane;             // logical column of the lane's first node
   const bool col_out = lane >= 1 && lane <= 30 && lxa < xend;
-  int xa = lxa % nx;                                     // every lane is a valid periodic pair
+  int xa = lxa % nx;                                     // every lane is a valid periodic group
   if (xa < 0) xa += nx;
-  // lanes whose pairs share a 32-byte sector of a population plane (rows keep the sector phase only
+  // lanes whose groups share a 32-byte sector of a population plane (rows keep the sector phase only
   // if the row pitch is a multiple of 32 bytes); a sector that holds any fluid node is stored whole
   // (zeros on its solid nodes), so that HBM never has to read-modify-write a partial sector
-  const int sector = (lxa + 64) * (int)sizeof(R) / 32;
+  const int sector = (lxa + 4 * NL) * (int)sizeof(R) / 32;
   const unsigned gmask = (LBM_PAIR_FULLSECTOR && (nx * (int)sizeof(R)) % 32 == 0) ? __match_any_sync(FULL, sector) : (1u << lane);
   const int j0 = blockIdx.y * TY;
   const int rows = min(TY, ny - j0);
@@ -155,18 +231,23 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   };
   auto inc = [](int v, int mod) { return v + 1 == mod ? 0 : v + 1; };
   // ---- asynchronous fetches (slots and row offsets are passed in: no modulo in the march) ----
-  auto issue_cls = [&](unsigned u, int sc) {   // the two class words of the pair (one aligned 4-byte word)
-    cp_async_vec<4>(sC0 + (unsigned)sc * C_STAGE, cl16 + (u + (unsigned)xa));
+  auto issue_cls = [&](unsigned u, int sc) {   // the NL class words of the lane (one aligned word)
+    cp_async_vec<NL * 2>(sC0 + (unsigned)sc * C_STAGE, cl16 + (u + (unsigned)xa));
   };
   // own-position populations and phi of one march row; lower/upper: the row feeds c_y <= 0 / c_y >= 0
   auto issue_row = [&](unsigned u, int sn, int sp, int sc, bool lower, bool upper) {
-    const unsigned w2 = S.Cw[sc][lane];
-    const unsigned ca = w2 & 0xffu, cb = (w2 >> 16) & 0xffu;
+    unsigned cmin = 3u, cmax = 0u;   // classes: 0,1 fluid; 2 ghost; 3 bulk solid
+#pragma unroll
+    for (int c = 0; c < NL; c++) {
+      const unsigned cc = S.Cw[sc][lane][c] & 0xffu;
+      cmin = min(cmin, cc);
+    }
+    (void)cmax;
     const unsigned k = u + (unsigned)xa;
-    if (ca != 3u || cb != 3u) cp_async_vec<VB>(sP0 + (unsigned)sp * P_STAGE, phi_in + k);
-    if (ca < 2u || cb < 2u) {
+    if (cmin != 3u) cp_async_vec<VB>(sP0 + (unsigned)sp * P_STAGE, phi_in + k);
+    if (cmin < 2u) {
       const unsigned d = sN0 + (unsigned)sn * N_STAGE;
-      const char* src = reinterpret_cast<const char*>(Nsrc + k);   // plane q is src + q * psB: one IMAD.WIDE each
+      const char* src = reinterpret_cast<const char*>(Nsrc + k);   // plane q is src + q * psB
       if (lower && upper) {
         cp_async_vec<VB>(d + 0 * N_PLANE, src);
         cp_async_vec<VB>(d + 1 * N_PLANE, src + (size_t)psB * 1u);
@@ -186,14 +267,14 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   };
 
   // ---- prologue: ring slot of march row m is (m + 1) mod ring size ----
+  const V zero = splat<V>(R(0));
   {   // stale ring entries are read (and discarded) for solid nodes: they must be finite
-    const V z = mk(R(0), R(0));
 #pragma unroll
     for (int s = 0; s < NS; s++)
 #pragma unroll
-      for (int q = 0; q < 9; q++) S.N[s][q][lane] = z;
+      for (int q = 0; q < 9; q++) S.N[s][q][lane] = zero;
 #pragma unroll
-    for (int s = 0; s < PS; s++) S.P[s][lane] = z;
+    for (int s = 0; s < PS; s++) S.P[s][lane] = zero;
   }
   for (int m = -1; m <= 2 * DP; m++)
     if (m <= last + 1) issue_cls((unsigned)wrap_row(m) * (unsigned)nx, (m + 1) % CS);
@@ -211,10 +292,11 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   int sP_a = 0, sP_b = 1, sP_c = 2, sP_f = (DP + 2) % PS;
   int sC_i = 1 % CS, sC_f = (DP + 2) % CS, sC_n = (2 * DP + 2) % CS;
   int rf = wrap_row(DP + 1), rc = wrap_row(2 * DP + 1);
-  unsigned kout = (unsigned)(j0 - 1) * (unsigned)nx + (unsigned)xa;   // own pair of march row i (1 <= i <= rows)
-  const V zero = mk(R(0), R(0));
+  unsigned kout = (unsigned)(j0 - 1) * (unsigned)nx + (unsigned)xa;   // own group of march row i (1 <= i <= rows)
   V acc_prev = zero, up_prev = zero;
-  bool fa_prev = false, fb_prev = false;
+  bool fl_prev[NL];
+#pragma unroll
+  for (int c = 0; c < NL; c++) fl_prev[c] = false;
 
   for (int i = 0; i <= last; i++) {
     cp_async_wait<DP - 1>();   // row i+1 and the class words of row i+1+DP have landed
@@ -227,14 +309,22 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     cp_async_commit();
 
     // ---- on-chip operands of march row i ----
-    const unsigned w2 = S.Cw[sC_i][lane];
     const V A0 = S.N[sN_b][0][lane], A1 = S.N[sN_b][1][lane], A3 = S.N[sN_b][3][lane];
     const V Cn0 = S.N[sN_c][4][lane], Cn1 = S.N[sN_c][7][lane], Cn2 = S.N[sN_c][8][lane];
     const V pC = S.P[sP_b][lane], pN = S.P[sP_c][lane];
 
-    const bool fa = (w2 & 0xffu) < 2u, fb = ((w2 >> 16) & 0xffu) < 2u;
-    const unsigned lka = fa ? (w2 >> 8) & 0xffu : 0u, lkb = fb ? (w2 >> 24) : 0u;
-    const bool any_link = __any_sync(FULL, (lka | lkb) != 0u);
+    bool fl[NL];
+    unsigned lk[NL];
+    bool any_fl = false, all_fl = true;
+    unsigned lk_any = 0u;
+#pragma unroll
+    for (int c = 0; c < NL; c++) {
+      const unsigned w = S.Cw[sC_i][lane][c];
+      fl[c] = (w & 0xffu) < 2u;
+      lk[c] = fl[c] ? (w >> 8) : 0u;
+      any_fl |= fl[c]; all_fl &= fl[c]; lk_any |= lk[c];
+    }
+    const bool any_link = __any_sync(FULL, lk_any != 0u);
 
     // pulled populations: propagation A16-A17 on chip
     V nn[9];
@@ -246,26 +336,27 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
                         S.N[sN_b][6][lane], S.N[sN_b][7][lane], S.N[sN_b][8][lane]};   // plane q at (x, i)
 #pragma unroll
       for (int q = 1; q < 9; q++) {
-        const V o = own[opp(q)];
-        R a = lo(nn[q]), b = hi(nn[q]);
-        if ((lka >> (q - 1)) & 1u) a = lo(o);
-        if ((lkb >> (q - 1)) & 1u) b = hi(o);
-        nn[q] = mk(a, b);
+        R a[NL], o[NL];
+        L::unpack(nn[q], a);
+        L::unpack(own[opp(q)], o);
+#pragma unroll
+        for (int c = 0; c < NL; c++)
+          if ((lk[c] >> (q - 1)) & 1u) a[c] = o[c];
+        nn[q] = L::pack(a);
       }
     }
-    const unsigned fmask = __ballot_sync(FULL, col_out && (fa || fb));
+    const unsigned fmask = __ballot_sync(FULL, col_out && any_fl);
     const bool st = col_out && i >= 1 && i <= rows && (fmask & gmask) != 0u;   // my sector holds a fluid node
-
     // phi stencil (R8): west / east neighbours of the three rows (shuffles: all lanes take part)
     const V pCw = from_left(pC), pCe = from_right(pC), pNw = from_left(pN), pNe = from_right(pN);
     const V pSw = from_left(pS), pSe = from_right(pS);
 
     V bs[9];
     V bb = zero;
-    if (fa || fb || st) {   // st without a fluid node: a solid pair completing a sector with zeros
+    if (any_fl || st) {   // st without a fluid node: a solid group completing a sector with zeros
       const V ph[9] = {pC, pCe, pN, pCw, pS, pNe, pNw, pSw, pSe};
       V ns[9];
-      collide_pair<R, V>(C, nn, ph, fa, fb, ns, bs);
+      collide_lane<V>(C, nn, ph, fl, all_fl, ns, bs);
       if (st) {
         char* dst = reinterpret_cast<char*>(Ndst + kout);
 #pragma unroll
@@ -276,14 +367,19 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dstB + (size_t)psB * (unsigned)q) = bs[q];
         }
       }
-      if (lka | lkb) {   // link q hands the node its own B_opp(q)* back
-        R ba = R(0), bbv = R(0);
+      if (lk_any) {   // link q hands the node its own B_opp(q)* back
+        R b[NL];
+#pragma unroll
+        for (int c = 0; c < NL; c++) b[c] = R(0);
 #pragma unroll
         for (int q = 1; q < 9; q++) {
-          if ((lka >> (q - 1)) & 1u) ba += lo(bs[opp(q)]);
-          if ((lkb >> (q - 1)) & 1u) bbv += hi(bs[opp(q)]);
+          R o[NL];
+          L::unpack(bs[opp(q)], o);
+#pragma unroll
+          for (int c = 0; c < NL; c++)
+            if ((lk[c] >> (q - 1)) & 1u) b[c] += o[c];
         }
-        bb = mk(ba, bbv);
+        bb = L::pack(b);
       }
     } else {
 #pragma unroll
@@ -296,15 +392,22 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     if (i >= 2 && col_out) {
       const V pn = acc_prev + down;
       R* dst = phi_out + (kout - (unsigned)nx);
-      if (fa_prev && fb_prev) *reinterpret_cast<V*>(dst) = pn;
+      bool allp = true;
+#pragma unroll
+      for (int c = 0; c < NL; c++) allp &= fl_prev[c];
+      if (allp) *reinterpret_cast<V*>(dst) = pn;
       else {
-        if (fa_prev) dst[0] = lo(pn);
-        if (fb_prev) dst[1] = hi(pn);
+        R x[NL];
+        L::unpack(pn, x);
+#pragma unroll
+        for (int c = 0; c < NL; c++)
+          if (fl_prev[c]) dst[c] = x[c];
       }
     }
     acc_prev = (up_prev + mid) + bb;
     up_prev = upw;
-    fa_prev = fa; fb_prev = fb;
+#pragma unroll
+    for (int c = 0; c < NL; c++) fl_prev[c] = fl[c];
 
     kout += (unsigned)nx;
     sN_a = sN_b; sN_b = sN_c; sN_c = inc(sN_c, NS);
@@ -315,28 +418,20 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   cp_async_wait<0>();
 }
 
-template <typename R>
-struct PairCfg {
-  static constexpr int DP = sizeof(R) == 8 ? LBM_PAIR_DP64 : LBM_PAIR_DP32;
-  static constexpr int WARPS = LBM_PAIR_WARPS;
-  static constexpr int MINB = sizeof(R) == 8 ? LBM_PAIR_MINB64 : LBM_PAIR_MINB32;
-};
-
-// returns false if the grid does not fit the schedule (odd nx): the caller uses another schedule
-template <typename R>
-bool launch_fused_pair(const Consts<R>& C, const uint16_t* cl16, const R* Nsrc, R* Ndst, R* Bdst,
-                       const R* phi_in, R* phi_out, cudaStream_t st) {
-  using Cfg = PairCfg<R>;
-  constexpr int DP = Cfg::DP, WARPS = Cfg::WARPS, MINB = Cfg::MINB;
-  if (C.nx & 1) return false;
-  const int nwx = (C.nx + 59) / 60;
+template <typename V, int DP, int MINB>
+bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* cl16,
+                       const typename LaneOf<V>::R* Nsrc, typename LaneOf<V>::R* Ndst, typename LaneOf<V>::R* Bdst,
+                       const typename LaneOf<V>::R* phi_in, typename LaneOf<V>::R* phi_out, cudaStream_t st) {
+  constexpr int WARPS = LBM_PAIR_WARPS;
+  constexpr int OUTC = 30 * LaneOf<V>::NL;
+  const int nwx = (C.nx + OUTC - 1) / OUTC;
   const int gx = (nwx + WARPS - 1) / WARPS;
   // rows per warp march: long marches amortise the halo rows; small grids need enough CTAs
   int TY = LBM_PAIR_TY;
   while (TY > 8 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 8) TY >>= 1;
   const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
-  const size_t smem = sizeof(PairRing<R, DP>) * WARPS;
-  auto kern = Bdst ? k_fused_pair<R, DP, WARPS, MINB, true> : k_fused_pair<R, DP, WARPS, MINB, false>;
+  const size_t smem = sizeof(PairRing<V, DP>) * WARPS;
+  auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true> : k_fused_pair<V, DP, WARPS, MINB, false>;
   static bool attr_set[2] = {false, false};
   if (!attr_set[Bdst ? 1 : 0]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
@@ -344,6 +439,20 @@ bool launch_fused_pair(const Consts<R>& C, const uint16_t* cl16, const R* Nsrc, 
   }
   kern<<<grid, 32 * WARPS, smem, st>>>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, TY);
   return true;
+}
+
+// returns false if the grid does not fit the schedule (odd nx): the caller uses another schedule
+inline bool launch_fused_pair(const Consts<double>& C, const uint16_t* cl16, const double* Nsrc, double* Ndst,
+                              double* Bdst, const double* phi_in, double* phi_out, cudaStream_t st) {
+  if (C.nx & 1) return false;
+  return launch_fused_lane<D2, LBM_PAIR_DP64, LBM_PAIR_MINB64>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
+}
+inline bool launch_fused_pair(const Consts<float>& C, const uint16_t* cl16, const float* Nsrc, float* Ndst,
+                              float* Bdst, const float* phi_in, float* phi_out, cudaStream_t st) {
+  if (C.nx & 1) return false;
+  if (LBM_PAIR_QUAD && (C.nx & 3) == 0)
+    return launch_fused_lane<Q4, LBM_PAIR_DP32, LBM_PAIR_MINBQ>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
+  return launch_fused_lane<F2, LBM_PAIR_DP32, LBM_PAIR_MINB32>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
 }
 
 }  // namespace lbm

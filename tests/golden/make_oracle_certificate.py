@@ -24,9 +24,11 @@ from paper_2605_30878_b200 import workloads as wl  # noqa: E402
 def main():
     cert = {"source": "oracle/lbmref.c via tests/golden/make_oracle_certificate.py",
             "contact_angle": [], "laplace": []}
-    # config 2 geometry at half scale (128^2, R = 20, drop 17.5, W = 5), 20,000 steps
-    for theta in (30.0, 60.0, 90.0, 120.0, 150.0):
-        w = wl.config2(seed=0, theta_deg=theta, n=128)
+    # config 2 geometry at half scale (128^2, R = 20, drop 17.5, W = 5), 20,000 steps; at 30 deg the
+    # cap is so flat that no contour point lies farther than 2W from the solid at that scale, so
+    # that angle runs at full scale (256^2, R = 40)
+    for theta, n in ((30.0, 256), (60.0, 128), (90.0, 128), (120.0, 128), (150.0, 128)):
+        w = wl.config2(seed=0, theta_deg=theta, n=n)
         s = ref.RefLBM(ref.RefParams(**w.param_dict()), w.mask, w.disks)
         s.init(w.phi0)
         m0 = s.diag()["sum_phi"]
