@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <new>
+#include <vector>
 
 #include "../../include/lbm.h"
 #include "lbm_fused.cuh"
@@ -129,6 +130,40 @@ int check_walls(const lbm_params* P, const uint8_t* mask) {
 size_t plane_stride(const lbm_params* P) {
   const size_t n = (size_t)P->nx * P->ny;
   return ((n + 63) & ~(size_t)63) + 37 * 64;
+}
+
+// Uniform grid of disk candidates for the one-time ghost geometry: cell (cy, cx) lists, in increasing
+// disk index, every disk whose periodic bounding box overlaps the cell.
+constexpr int kCell = 64;
+void cover_cells(double lo, double hi, int n, int nc, std::vector<char>& hit) {
+  std::fill(hit.begin(), hit.end(), 0);
+  if (hi - lo >= n) { std::fill(hit.begin(), hit.end(), 1); return; }
+  // walk the interval cell by cell in unwrapped coordinates; wrap every probe point
+  for (double x = floor(lo); x <= floor(hi) + 1; x += 1.0) {
+    if (x < floor(lo) || x > ceil(hi)) continue;
+    long long xi = (long long)x % n;
+    if (xi < 0) xi += n;
+    hit[(size_t)(xi / kCell) < (size_t)nc ? xi / kCell : nc - 1] = 1;
+  }
+}
+void build_disk_cells(const lbm_params* P, const lbm_disk* disks, int n_disks, int* ncx_out,
+                      std::vector<int>& start, std::vector<int>& list) {
+  const int ncx = (P->nx + kCell - 1) / kCell, ncy = (P->ny + kCell - 1) / kCell;
+  *ncx_out = ncx;
+  std::vector<std::vector<int>> cells((size_t)ncx * ncy);
+  std::vector<char> hx(ncx), hy(ncy);
+  for (int d = 0; d < n_disks; d++) {
+    cover_cells(disks[d].cx - disks[d].r - 1.0, disks[d].cx + disks[d].r + 1.0, P->nx, ncx, hx);
+    cover_cells(disks[d].cy - disks[d].r - 1.0, disks[d].cy + disks[d].r + 1.0, P->ny, ncy, hy);
+    for (int cy = 0; cy < ncy; cy++)
+      if (hy[cy])
+        for (int cx = 0; cx < ncx; cx++)
+          if (hx[cx]) cells[(size_t)cy * ncx + cx].push_back(d);
+  }
+  start.assign(cells.size() + 1, 0);
+  for (size_t k = 0; k < cells.size(); k++) start[k + 1] = start[k] + (int)cells[k].size();
+  list.resize((size_t)start.back() + 1);
+  for (size_t k = 0; k < cells.size(); k++) std::copy(cells[k].begin(), cells[k].end(), list.begin() + start[k]);
 }
 
 bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELINE; }
@@ -389,18 +424,31 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     if (n_disks > 0) CKC(cudaMemcpyAsync(d_disks, disks, disk_bytes, cudaMemcpyHostToDevice, c->st));
     CKC(cudaMemsetAsync(c->scal + 1, 0, sizeof(int), c->st));
     const unsigned gb = (unsigned)((ng + 127) / 128);
+    int ncx = 1;
+    std::vector<int> h_start, h_list;
+    build_disk_cells(prm, disks, n_disks, &ncx, h_start, h_list);
+    int* d_cells = nullptr;   // [start | list], freed after the geometry kernel
+    CKC(cudaMalloc(&d_cells, (h_start.size() + h_list.size()) * sizeof(int)));
+    int* d_start = d_cells;
+    int* d_list = d_cells + h_start.size();
+    cudaMemcpyAsync(d_start, h_start.data(), h_start.size() * sizeof(int), cudaMemcpyHostToDevice, c->st);
+    cudaMemcpyAsync(d_list, h_list.data(), h_list.size() * sizeof(int), cudaMemcpyHostToDevice, c->st);
     if (c->is32)
       k_ghost_geometry<float><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
-                                                     n_disks, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
+                                                     n_disks, d_start, d_list, ncx, kCell, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
                                                      c->wgt_d, (float*)c->wgt, c->csolid, c->scal + 1);
     else
       k_ghost_geometry<double><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
-                                                      n_disks, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
+                                                      n_disks, d_start, d_list, ncx, kCell, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
                                                       c->wgt_d, (double*)c->wgt, c->csolid, c->scal + 1);
     CKC(cudaGetLastError());
     int bad = 0;
-    CKC(cudaMemcpyAsync(&bad, c->scal + 1, sizeof(int), cudaMemcpyDeviceToHost, c->st));
-    CKC(cudaStreamSynchronize(c->st));
+    cudaMemcpyAsync(&bad, c->scal + 1, sizeof(int), cudaMemcpyDeviceToHost, c->st);
+    {
+      const cudaError_t e = cudaStreamSynchronize(c->st);
+      cudaFree(d_cells);
+      if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "ghost geometry"); }
+    }
     if (bad) {
       delete c;
       return fail(nullptr, LBM_EINVAL, "mask and geometry disagree: a ghost node lies in no disk");

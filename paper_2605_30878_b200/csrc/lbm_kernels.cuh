@@ -164,6 +164,8 @@ template <typename R>
 __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __restrict__ gidx, int nx,
                                                         int ny, int wall_rows,
                                                         const Disk* __restrict__ disks, int n_disks,
+                                                        const int* __restrict__ cell_start,
+                                                        const int* __restrict__ cell_disks, int ncx, int cell_size,
                                                         const uint8_t* __restrict__ cls,
                                                         double* __restrict__ gnx, double* __restrict__ gny,
                                                         double* __restrict__ gdepth,
@@ -181,9 +183,12 @@ __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __res
     depth = 0.5;  // half-way wall (R17)
     found = 1;
   } else {
+    // candidates: the disks whose bounding box overlaps this node's cell, in increasing disk index
+    // (so that "least depth, first wins ties" (R17) is the same as a scan over all disks)
     double best = 0.0;
-    for (int d = 0; d < n_disks; d++) {
-      const Disk dk = disks[d];
+    const int cell = (j / cell_size) * ncx + (i / cell_size);
+    for (int t = cell_start[cell]; t < cell_start[cell + 1]; t++) {
+      const Disk dk = disks[cell_disks[t]];
       const double dx = minimg_d(__dsub_rn((double)i, dk.cx), (double)nx);
       const double dy = minimg_d(__dsub_rn((double)j, dk.cy), (double)ny);
       const double r2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));

@@ -141,6 +141,25 @@ __device__ __forceinline__ V splat(typename LaneOf<V>::R s) {
   return L::pack(x);
 }
 
+#ifndef LBM_PAIR_STORE_CS
+#define LBM_PAIR_STORE_CS 0
+#endif
+// vector store of a lane's NL values; optionally with the streaming (evict-first) cache hint
+template <typename V>
+__device__ __forceinline__ void store_vec(void* p, V v) {
+#if LBM_PAIR_STORE_CS
+  if constexpr (sizeof(V) == 8) {
+    const float2 t = *reinterpret_cast<const float2*>(&v);
+    __stcs(reinterpret_cast<float2*>(p), t);
+  } else {
+    const float4 t = *reinterpret_cast<const float4*>(&v);
+    __stcs(reinterpret_cast<float4*>(p), t);
+  }
+#else
+  *reinterpret_cast<V*>(p) = v;
+#endif
+}
+
 template <int BYTES>
 __device__ __forceinline__ void cp_async_vec(unsigned saddr, const void* gptr) {
   // .ca for every size: with .cg (L1 bypass) the two 16-byte lanes of a sector each fetch it from L2
@@ -360,7 +379,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       if (st) {
         char* dst = reinterpret_cast<char*>(Ndst + kout);
 #pragma unroll
-        for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dst + (size_t)psB * (unsigned)q) = ns[q];
+        for (int q = 0; q < 9; q++) store_vec<V>(dst + (size_t)psB * (unsigned)q, ns[q]);
         if (WRITE_B) {
           char* dstB = reinterpret_cast<char*>(Bdst + kout);
 #pragma unroll
@@ -395,7 +414,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       bool allp = true;
 #pragma unroll
       for (int c = 0; c < NL; c++) allp &= fl_prev[c];
-      if (allp) *reinterpret_cast<V*>(dst) = pn;
+      if (allp) store_vec<V>(dst, pn);
       else {
         R x[NL];
         L::unpack(pn, x);
