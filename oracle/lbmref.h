@@ -78,6 +78,10 @@ void   lbmref_bilinear_setup(double xF, double yF, int32_t nx, int32_t ny,
 void   lbmref_node_update(const lbmref_params* prm, const double N[9], const double phi_nb[9],
                           double Nstar[9], double Bstar[9], lbmref_node_fields* f);
 
+/* NEXT row f2: unit solid normal from the mask alone (indicator smoothed twice, sixth-order isotropic stencil) */
+void lbmref_mask_smooth(const int32_t* in, int32_t* out, int nx, int ny);
+void lbmref_mask_normal(const int32_t* s, int nx, int ny, int i, int j, double* nxs, double* nys);
+
 #ifdef __cplusplus
 }
 #endif

@@ -433,13 +433,20 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     int* d_list = d_cells + h_start.size();
     cudaMemcpyAsync(d_start, h_start.data(), h_start.size() * sizeof(int), cudaMemcpyHostToDevice, c->st);
     cudaMemcpyAsync(d_list, h_list.data(), h_list.size() * sizeof(int), cudaMemcpyHostToDevice, c->st);
+    int* d_smooth = nullptr;   // mask-only normals (n_disks == 0): the solid indicator smoothed twice
+    if (n_disks == 0) {
+      cudaError_t e = cudaMalloc(&d_smooth, 2 * n * sizeof(int));
+      if (e != cudaSuccess) { cudaFree(d_cells); delete c; return cuda_fail(nullptr, e, "cudaMalloc(mask normals)"); }
+      k_mask_smooth<<<nblk, 256, 0, c->st>>>(c->cls, nullptr, d_smooth + n, prm->nx, prm->ny);
+      k_mask_smooth<<<nblk, 256, 0, c->st>>>(nullptr, d_smooth + n, d_smooth, prm->nx, prm->ny);
+    }
     if (c->is32)
       k_ghost_geometry<float><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
-                                                     n_disks, d_start, d_list, ncx, kCell, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
+                                                     n_disks, d_start, d_list, ncx, kCell, d_smooth, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
                                                      c->wgt_d, (float*)c->wgt, c->csolid, c->scal + 1);
     else
       k_ghost_geometry<double><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
-                                                      n_disks, d_start, d_list, ncx, kCell, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
+                                                      n_disks, d_start, d_list, ncx, kCell, d_smooth, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
                                                       c->wgt_d, (double*)c->wgt, c->csolid, c->scal + 1);
     CKC(cudaGetLastError());
     int bad = 0;
@@ -447,6 +454,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     {
       const cudaError_t e = cudaStreamSynchronize(c->st);
       cudaFree(d_cells);
+      cudaFree(d_smooth);
       if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "ghost geometry"); }
     }
     if (bad) {

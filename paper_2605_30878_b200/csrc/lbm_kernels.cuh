@@ -149,6 +149,32 @@ __global__ void __launch_bounds__(256) k_compact_ghosts(const uint8_t* __restric
 // that the list can be compared bit for bit.
 struct Disk { double cx, cy, r; };
 
+// one smoothing pass of the solid indicator for the mask-only normals (NEXT row f2): centre weight
+// 60 and the sixth-order isotropic weights 32, 12, 1 (x120) at |c|^2 = 1, 2, 4; integers, periodic.
+// from_cls: the input is the class array (solid <=> class >= 2) instead of an int field.
+__global__ void __launch_bounds__(256) k_mask_smooth(const uint8_t* __restrict__ cls, const int* __restrict__ in,
+                                                     int* __restrict__ out, int nx, int ny) {
+  const long long k = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (k >= (long long)nx * ny) return;
+  const int i = (int)(k % nx), j = (int)(k / nx);
+  const int ox[12] = {1, 0, -1, 0, 1, -1, -1, 1, 2, 0, -2, 0};
+  const int oy[12] = {0, 1, 0, -1, 1, 1, -1, -1, 0, 2, 0, -2};
+  const int wg[12] = {32, 32, 32, 32, 12, 12, 12, 12, 1, 1, 1, 1};
+  auto val = [&](int ii, int jj) -> int {
+    const long long q = (long long)jj * nx + ii;
+    return cls ? (cls[q] >= 2 ? 1 : 0) : in[q];
+  };
+  int acc = 60 * val(i, j);
+#pragma unroll
+  for (int t = 0; t < 12; t++) {
+    int ii = i + ox[t], jj = j + oy[t];
+    ii = ii < 0 ? ii + nx : (ii >= nx ? ii - nx : ii);
+    jj = jj < 0 ? jj + ny : (jj >= ny ? jj - ny : jj);
+    acc += wg[t] * val(ii, jj);
+  }
+  out[k] = acc;
+}
+
 __device__ __forceinline__ double minimg_d(double d, double L) {
   d = fmod(d, L);
   if (d >= 0.5 * L) d = __dsub_rn(d, L);
@@ -166,6 +192,7 @@ __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __res
                                                         const Disk* __restrict__ disks, int n_disks,
                                                         const int* __restrict__ cell_start,
                                                         const int* __restrict__ cell_disks, int ncx, int cell_size,
+                                                        const int* __restrict__ smooth2,
                                                         const uint8_t* __restrict__ cls,
                                                         double* __restrict__ gnx, double* __restrict__ gny,
                                                         double* __restrict__ gdepth,
@@ -204,6 +231,27 @@ __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __res
         }
       }
     }
+  }
+  if (!found && n_disks == 0 && smooth2 != nullptr) {
+    // NEXT row f2: no analytic shape was given.  Normal from the mask alone: minus the
+    // sixth-order isotropic gradient (12 points, weights x120 = 32, 12, 1: exact integer sums) of the
+    // solid indicator smoothed twice (k_mask_smooth); (0,0) where it vanishes.
+    const int ox[12] = {1, 0, -1, 0, 1, -1, -1, 1, 2, 0, -2, 0};
+    const int oy[12] = {0, 1, 0, -1, 1, 1, -1, -1, 0, 2, 0, -2};
+    const int wg[12] = {32, 32, 32, 32, 12, 12, 12, 12, 1, 1, 1, 1};
+    long long gxs = 0, gys = 0;
+#pragma unroll
+    for (int t = 0; t < 12; t++) {
+      const int ii = wrapi_d(i + ox[t], nx), jj = wrapi_d(j + oy[t], ny);
+      const long long v = smooth2[jj * nx + ii];
+      gxs += (long long)(wg[t] * ox[t]) * v;
+      gys += (long long)(wg[t] * oy[t]) * v;
+    }
+    const double ax = -(double)gxs, ay = -(double)gys;
+    const double m = __dsqrt_rn(__dadd_rn(__dmul_rn(ax, ax), __dmul_rn(ay, ay)));
+    if (m > 0.0) { nxs = __ddiv_rn(ax, m); nys = __ddiv_rn(ay, m); }
+    depth = 0.0;
+    found = 1;
   }
   if (!found) atomicExch(err, 1);
   gnx[g] = nxs; gny[g] = nys; gdepth[g] = depth;

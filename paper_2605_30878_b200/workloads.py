@@ -255,3 +255,35 @@ def flat_interface(nx: int, ny: int, W: float = 4.0):
     y = np.arange(ny, dtype=np.float64)
     prof = 0.5 * (np.tanh(2.0 * (y - 0.25 * ny) / W) - np.tanh(2.0 * (y - 0.75 * ny) / W))
     return np.zeros((ny, nx), np.uint8), np.zeros((0, 3)), np.repeat(prof[:, None], nx, axis=1)
+
+
+# ---- NEXT row f3: drop on a flat plate (§III.A, :102-124) -----------------------------------
+def flat_plate(theta_deg: float = 60.0, W: float = 4.0, scale: float = 1.0, rho_ratio: float = 1000.0,
+               mu_ratio: float = 100.0, sigma: float = 1e-2, x_offset: float = 0.0) -> Workload:
+    """Drop of area A = 1e4 scale^2 on the bottom wall of a (500, 300) scale box, periodic in x, wall rows
+    at j = 0 and j = ny-1 (+2 wall rows as in the paper's Table I grids).  The drop starts
+    as the analytic circular cap of the prescribed angle (:114): R_c = sqrt(2A / (2 theta - sin 2 theta)),
+    centre at height -R_c cos(theta) relative to the wall surface, which lies half-way between the wall row
+    and the first fluid row (R12, R17).  x_offset shifts the drop off the lattice symmetry axis: on a mirror-symmetric
+    set-up grad(phi) cancels to round-off at the centre of curvature, where the direction of n_phi (R16) is
+    then decided by rounding order, so element-wise parity runs use an offset."""
+    nx = int(round(500 * scale))
+    nx += nx & 1
+    ny = int(round(300 * scale)) + 2
+    A = 1.0e4 * scale * scale
+    th = math.radians(theta_deg)
+    Rc = math.sqrt(2.0 * A / (2.0 * th - math.sin(2.0 * th)))
+    y_wall = 0.5
+    cx, cy = 0.5 * nx + x_offset, y_wall - Rc * math.cos(th)
+    mask = np.zeros((ny, nx), dtype=np.uint8)
+    mask[0, :] = 1
+    mask[ny - 1, :] = 1
+    yy, xx = np.mgrid[0:ny, 0:nx].astype(np.float64)
+    r = np.hypot(xx - cx, yy - cy)
+    phi0 = 0.5 * (1.0 - np.tanh(2.0 * (r - Rc) / W))
+    nu_l, nu_g = viscosities(rho_ratio, mu_ratio)
+    w = Workload(f"flat_plate_{nx}x{ny}_theta{theta_deg:g}_W{W:g}", nx, ny, mask, np.zeros((0, 3)), phi0,
+                 rho_l=rho_ratio * RHO_G, rho_g=RHO_G, nu_l=nu_l, nu_g=nu_g, sigma=sigma, W=W,
+                 theta_deg=theta_deg, wall_rows=1, steps=20000, seed=0)
+    w.meta.update(area=A, Rc=Rc, y_wall=y_wall)
+    return w

@@ -97,3 +97,20 @@ def analytic_drop_on_cylinder(R: float, A: float, theta_deg: float):
     Rc = 0.5 * (lo + hi)
     d = math.sqrt(R * R + Rc * Rc - 2 * R * Rc * ct)
     return Rc, d, d + Rc
+
+
+def contact_angle_on_plate(phi: np.ndarray, mask: np.ndarray, W: float, y_wall: float = 0.5, exclude: float = 2.0):
+    """(theta_m in degrees, spread S, height H) of a drop on the bottom wall, Eq. 12 (:118):
+    theta_m = arccos((S^2 - H^2) / (S^2 + H^2)) with S the HALF spread on the wall and H the apex height.
+    S and H come from the circle fitted to the phi = 1/2 contour farther than `exclude` W from the wall
+    (the diffuse profile is distorted next to the wall), evaluated on the wall surface y_wall."""
+    pts = half_contour_points(phi, mask)
+    pts = pts[pts[:, 1] > y_wall + exclude * W]
+    if len(pts) < 8:
+        raise ValueError("too few contour points")
+    cx, cy, Rc = fit_circle(pts)
+    h = cy - y_wall                       # centre height above the wall (negative for theta < 90)
+    H = h + Rc
+    S = math.sqrt(max(Rc * Rc - h * h, 0.0))
+    theta = math.degrees(math.acos((S * S - H * H) / (S * S + H * H)))
+    return theta, S, H

@@ -337,3 +337,44 @@ def test_config5_8192_properties_and_samples():
         res[sched] = s.sample_populations(idx)[0]
         s.close()
     assert np.abs(res[0] - res[BASELINE]).max() <= 1e-13
+
+
+# ---- NEXT row f3: drop on a flat plate (§III.A): wall rows only, no disk list -------------
+@pytest.mark.parametrize("precision", [64, 32])
+def test_flat_plate_fields_and_eq12_angle(precision):
+    w = wl.flat_plate(theta_deg=120.0, W=4.0, scale=0.25, rho_ratio=10.0, mu_ratio=10.0, x_offset=0.37)
+    g, o = make_pair(w, precision=precision)
+    g.init(w.phi0); o.init(w.phi0)
+    g.step(500); o.step(500)
+    err, scale = field_errors(g, o)
+    tg = ms.contact_angle_on_plate(g.get()["phi"], w.mask, w.W)[0]
+    to = ms.contact_angle_on_plate(o.get()["phi"], w.mask, w.W)[0]
+    print("flat plate", precision, err, tg, to)
+    assert abs(tg - to) <= 0.5
+    if precision == 64:
+        assert max(err.values()) <= 1e-10, err
+    else:
+        uscale = max(scale["ux"], scale["uy"], w.sigma / (w.rho_l * w.nu_l))
+        assert err["phi"] <= 2e-4 and max(err["ux"], err["uy"]) <= 2e-4 * uscale
+
+
+# ---- NEXT row f2: geometry from the mask alone (no disk list) ------------------------------------------
+def test_mask_only_geometry_bit_exact_and_fields():
+    rng = np.random.default_rng(11)
+    n = 96
+    disks = np.array([[30.2, 40.7, 17.0], [70.5, 60.1, 11.5]])
+    mask = wl.rasterize_disks(n, n, disks)
+    mask[80:84, 10:50] = 1                                     # a bar: not describable by the disk list
+    yy, xx = np.mgrid[0:n, 0:n]
+    phi0 = 0.5 * (1 - np.tanh(2 * (np.hypot(xx - 48.3, yy - 22.7) - 14.0) / 4.0))   # off-lattice centre, see R16
+    w = ArrayWorkload(mask, phi0, theta_deg=65.0)
+    g, o = make_pair(w)
+    cg, co = g.get_classification(), o.get_classification()
+    assert np.array_equal(cg["cls"], co["cls"]) and np.array_equal(cg["idx"], co["idx"])
+    for k in ("nx", "ny", "depth"):
+        assert np.array_equal(cg[k], co[k]), k                 # bit-exact normals
+    assert np.array_equal(cg["corner"], co["corner"]) and np.array_equal(cg["wgt"], co["wgt"])
+    g.init(w.phi0); o.init(w.phi0)
+    g.step(50); o.step(50)
+    err, _ = field_errors(g, o)
+    assert max(err.values()) < 1e-12, err
