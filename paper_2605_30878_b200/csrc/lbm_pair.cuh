@@ -46,6 +46,9 @@ namespace lbm {
 #ifndef LBM_PAIR_FULLSECTOR
 #define LBM_PAIR_FULLSECTOR 1
 #endif
+#ifndef LBM_PAIR_SECTOR
+#define LBM_PAIR_SECTOR 32   // bytes of the write granule that is completed with zeros
+#endif
 #ifndef LBM_PAIR_TY
 #define LBM_PAIR_TY 64
 #endif
@@ -238,8 +241,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   // lanes whose groups share a 32-byte sector of a population plane (rows keep the sector phase only
   // if the row pitch is a multiple of 32 bytes); a sector that holds any fluid node is stored whole
   // (zeros on its solid nodes), so that HBM never has to read-modify-write a partial sector
-  const int sector = (lxa + 4 * NL) * (int)sizeof(R) / 32;
-  const unsigned gmask = (LBM_PAIR_FULLSECTOR && (nx * (int)sizeof(R)) % 32 == 0) ? __match_any_sync(FULL, sector) : (1u << lane);
+  const int sector = (lxa + 32 * NL) * (int)sizeof(R) / LBM_PAIR_SECTOR;
+  const unsigned gmask = (LBM_PAIR_FULLSECTOR && (nx * (int)sizeof(R)) % LBM_PAIR_SECTOR == 0) ? __match_any_sync(FULL, sector) : (1u << lane);
   const int j0 = blockIdx.y * TY;
   const int rows = min(TY, ny - j0);
   const int last = rows + 1;                             // march row m = grid row j0-1+m; collided: 0..last

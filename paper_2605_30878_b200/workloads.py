@@ -287,3 +287,27 @@ def flat_plate(theta_deg: float = 60.0, W: float = 4.0, scale: float = 1.0, rho_
                  theta_deg=theta_deg, wall_rows=1, steps=20000, seed=0)
     w.meta.update(area=A, Rc=Rc, y_wall=y_wall)
     return w
+
+
+def particle_at_interface(theta_deg: float = 60.0, R: float = 25.0, W: float = 4.0, rho_ratio: float = 10.0,
+                          mu_ratio: float = 10.0, sigma: float = 1e-2) -> Workload:
+    """Fixed cylinder of radius R at a flat liquid-gas interface (§III.C, :136-197): box
+    (4.8 R, 4.8 R), periodic in x, no-slip walls at top and bottom (+2 wall rows, cf. the 120 x 122 grid of
+    Table I), cylinder centred in the box, liquid below the line through its centre."""
+    L = int(round(4.8 * R))
+    L += L & 1
+    nx, ny = L, L + 2
+    y_wall = 0.5
+    cx, cy = 0.5 * nx, y_wall + 0.5 * L
+    disks = np.array([[cx, cy, R]])
+    mask = rasterize_disks(nx, ny, disks)
+    mask[0, :] = 1
+    mask[ny - 1, :] = 1
+    yy = np.arange(ny, dtype=np.float64)[:, None] + np.zeros((1, nx))
+    phi0 = 0.5 * (1.0 - np.tanh(2.0 * (yy - cy) / W))
+    nu_l, nu_g = viscosities(rho_ratio, mu_ratio)
+    w = Workload(f"particle_at_interface_{nx}x{ny}_theta{theta_deg:g}", nx, ny, mask, disks, phi0,
+                 rho_l=rho_ratio * RHO_G, rho_g=RHO_G, nu_l=nu_l, nu_g=nu_g, sigma=sigma, W=W,
+                 theta_deg=theta_deg, wall_rows=1, steps=40000, seed=0)
+    w.meta.update(L=float(L), R=R, y_interface0=cy)
+    return w

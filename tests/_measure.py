@@ -114,3 +114,43 @@ def contact_angle_on_plate(phi: np.ndarray, mask: np.ndarray, W: float, y_wall: 
     S = math.sqrt(max(Rc * Rc - h * h, 0.0))
     theta = math.degrees(math.acos((S * S - H * H) / (S * S + H * H)))
     return theta, S, H
+
+
+def eq13_hstar(L: float, R: float, theta_deg: float):
+    """PAPER.md Eq. 13 (:180-189): periodic array of fixed cylinders at an interface.  Unknowns R_c, psi,
+    beta from  R^2 (L/R sin b - sin b cos b - b) = R_c^2 (psi - sin psi cos psi),
+    2 R_c cos(b + theta) = L - 2 R cos b,  psi = pi/2 - (b + theta);  returns
+    (h* = R_c (1 - cos psi) - R sin b, R_c, psi, beta).  theta > 90 deg follows from exchanging the two
+    phases: h*(theta) = -h*(180 - theta); theta = 90 deg: flat interface, h* = 0."""
+    if abs(theta_deg - 90.0) < 1e-12:
+        return 0.0, math.inf, 0.0, 0.0
+    if theta_deg > 90.0:
+        h, Rc, psi, beta = eq13_hstar(L, R, 180.0 - theta_deg)
+        return -h, Rc, psi, beta
+    th = math.radians(theta_deg)
+
+    def resid(b):
+        psi = 0.5 * math.pi - (b + th)
+        Rc = (L - 2.0 * R * math.cos(b)) / (2.0 * math.cos(b + th))
+        return R * R * (L / R * math.sin(b) - math.sin(b) * math.cos(b) - b) - Rc * Rc * (psi - math.sin(psi) * math.cos(psi))
+
+    lo, hi = 1e-9, 0.5 * math.pi - th - 1e-9        # resid(lo) < 0 (no area displaced), resid(hi) > 0 (psi -> 0)
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if resid(mid) < 0.0:
+            lo = mid
+        else:
+            hi = mid
+    b = 0.5 * (lo + hi)
+    psi = 0.5 * math.pi - (b + th)
+    Rc = (L - 2.0 * R * math.cos(b)) / (2.0 * math.cos(b + th))
+    return Rc * (1.0 - math.cos(psi)) - R * math.sin(b), Rc, psi, b
+
+
+def interface_height_at_boundary(phi: np.ndarray, level: float = 0.5) -> float:
+    """y of the phi = level crossing along the periodic boundary column x = 0 (linear interpolation,
+    liquid below), the quantity h* of PAPER.md §III.C is measured from."""
+    col = phi[:, 0]
+    j = np.nonzero((col[:-1] >= level) & (col[1:] < level))[0]
+    j = j[len(j) // 2] if len(j) > 1 else j[0]
+    return float(j + (col[j] - level) / (col[j] - col[j + 1]))

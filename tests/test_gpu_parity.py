@@ -378,3 +378,17 @@ def test_mask_only_geometry_bit_exact_and_fields():
     g.step(50); o.step(50)
     err, _ = field_errors(g, o)
     assert max(err.values()) < 1e-12, err
+
+
+def test_particle_at_interface_fields():
+    """PAPER.md §III.C set-up (walls + one cylinder through a flat interface): short run against the oracle."""
+    w = wl.particle_at_interface(theta_deg=60.0)
+    for precision, tol in ((64, 1e-10), (32, 2e-4)):
+        g, o = make_pair(w, precision=precision)
+        g.init(w.phi0); o.init(w.phi0)
+        g.step(400); o.step(400)
+        err, scale = field_errors(g, o)
+        uscale = max(scale["ux"], scale["uy"], w.sigma / (w.rho_l * w.nu_l))
+        assert err["phi"] <= tol and max(err["ux"], err["uy"]) <= (tol if precision == 64 else tol * uscale), err
+        yg = ms.interface_height_at_boundary(g.get()["phi"]); yo = ms.interface_height_at_boundary(o.get()["phi"])
+        assert abs(yg - yo) <= (1e-9 if precision == 64 else 1e-3)

@@ -212,3 +212,20 @@ def test_drop_on_flat_plate_contact_angle(theta):
     print("flat plate", theta, th0, th, d["umax"])
     assert abs(th - theta) < 6.0
     assert abs(d["sum_phi"] - m0) < 1e-10 * m0 and d["nan"] == 0
+
+
+# ---- NEXT row f3, second workload: fixed particle at an interface, Eq. 13 (§III.C) ---------
+def test_eq13_solver_identities():
+    L, R = 120.0, 25.0
+    assert ms.eq13_hstar(L, R, 90.0)[0] == 0.0
+    for th in (30.0, 45.0, 60.0, 80.0):
+        h, Rc, psi, b = ms.eq13_hstar(L, R, th)
+        # the three equations hold; the arc meets the cylinder at the contact angle
+        assert abs(2 * Rc * math.cos(b + math.radians(th)) - (L - 2 * R * math.cos(b))) < 1e-9
+        assert abs(psi - (math.pi / 2 - b - math.radians(th))) < 1e-12
+        lhs = R * R * (L / R * math.sin(b) - math.sin(b) * math.cos(b) - b)
+        assert abs(lhs - Rc * Rc * (psi - math.sin(psi) * math.cos(psi))) < 1e-6
+        assert h > 0 and 0 < b < math.pi / 2 and ms.eq13_hstar(L, R, 180.0 - th)[0] == -h
+    # a more wetting cylinder pulls the contact line further up: |h*| grows as theta leaves 90 deg
+    hs = [ms.eq13_hstar(L, R, th)[0] for th in (80.0, 60.0, 45.0, 30.0)]
+    assert all(a < b for a, b in zip(hs, hs[1:]))
