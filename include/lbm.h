@@ -119,13 +119,14 @@ int lbm_sync(lbm_ctx* ctx);
 int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, double* p);
 
 /* Post-stream populations N_i(x, t), B_i(x, t) of the current time, HOST 9*nx*ny doubles each
- * (SoA), either may be NULL; zeros on solid nodes.  Under LBM_SCHEDULE_FUSED the B_i are not part
- * of the stored state: they are available right after lbm_init, and after lbm_step only if
- * lbm_keep_B(ctx, 1) was set before that step (else LBM_EINVAL for B != NULL).  Synchronises. */
+ * (SoA), either may be NULL; zeros on solid nodes.  Under every schedule but BASELINE (FUSED,
+ * WARP, PAIR, hence AUTO) the B_i are not part of the stored state: they are available right after
+ * lbm_init, and after lbm_step only if lbm_keep_B(ctx, 1) was set before that step (else
+ * LBM_EINVAL for B != NULL).  Synchronises. */
 int lbm_get_populations(lbm_ctx* ctx, double* N, double* B);
 
-/* FUSED schedule only: when on != 0 the last time step of every lbm_step call also writes the
- * post-collision B_i* to HBM (workspace is sized for it) so that lbm_get_populations can return
+/* FUSED / WARP / PAIR schedules: when on != 0 the last time step of every lbm_step call also
+ * writes the post-collision B_i* to HBM (workspace is sized for it) so that lbm_get_populations can return
  * B_i.  No effect on the arithmetic.  Ignored by the BASELINE schedule (B always stored). */
 int lbm_keep_B(lbm_ctx* ctx, int32_t on);
 

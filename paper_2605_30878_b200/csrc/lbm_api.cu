@@ -588,7 +588,7 @@ int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, doub
 int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   if (B && !ctx->B_valid)
-    return fail(ctx, LBM_EINVAL, "B is not stored under the FUSED schedule: call lbm_keep_B(ctx, 1) before lbm_step");
+    return fail(ctx, LBM_EINVAL, "B is not stored under this schedule: call lbm_keep_B(ctx, 1) before lbm_step");
   const size_t n = ctx->n;
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
@@ -621,7 +621,7 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
 int lbm_sample_populations(lbm_ctx* ctx, int64_t n_idx, const int64_t* idx, double* N, double* B) {
   if (!ctx || n_idx < 0 || (n_idx > 0 && !idx)) return fail(ctx, LBM_EINVAL, "bad argument");
   if (B && !ctx->B_valid)
-    return fail(ctx, LBM_EINVAL, "B is not stored under the FUSED schedule: call lbm_keep_B(ctx, 1) before lbm_step");
+    return fail(ctx, LBM_EINVAL, "B is not stored under this schedule: call lbm_keep_B(ctx, 1) before lbm_step");
   if ((size_t)n_idx > ctx->samp_cap || (size_t)n_idx * 9 > 5 * ctx->n) return fail(ctx, LBM_EINVAL, "too many samples");
   for (int64_t t = 0; t < n_idx; t++)
     if (idx[t] < 0 || (size_t)idx[t] >= ctx->n) return fail(ctx, LBM_EINVAL, "sample index out of range");

@@ -184,6 +184,9 @@ def test_certificate_file_matches_if_present():
         assert abs(row["theta_measured"] - row["theta_set"]) < row["tol_deg"]
     for row in cert.get("laplace", []):
         assert abs(row["ratio"] - 1) < row["tol"]
+    for row in cert.get("particle", []):                 # Eq. 13 (:180-189), within the paper's own error band (:197)
+        assert abs(row["hstar_measured"] - row["hstar_eq13"]) < row["tol_rel"] * abs(row["hstar_eq13"])
+        assert abs(row["mass_drift_rel"]) < 1e-9
 
 
 # ---- NEXT row f3: drop on a flat plate, contact angle by Eq. 12 (§III.A) -------------------
