@@ -290,7 +290,7 @@ def flat_plate(theta_deg: float = 60.0, W: float = 4.0, scale: float = 1.0, rho_
 
 
 def particle_at_interface(theta_deg: float = 60.0, R: float = 25.0, W: float = 4.0, rho_ratio: float = 10.0,
-                          mu_ratio: float = 10.0, sigma: float = 1e-2) -> Workload:
+                          mu_ratio: float = 10.0, sigma: float = 1e-2, x_offset: float = 0.0) -> Workload:
     """Fixed cylinder of radius R at a flat liquid-gas interface (§III.C, :136-197): box
     (4.8 R, 4.8 R), periodic in x, no-slip walls at top and bottom (+2 wall rows, cf. the 120 x 122 grid of
     Table I), cylinder centred in the box, liquid below the line through its centre."""
@@ -298,7 +298,7 @@ def particle_at_interface(theta_deg: float = 60.0, R: float = 25.0, W: float = 4
     L += L & 1
     nx, ny = L, L + 2
     y_wall = 0.5
-    cx, cy = 0.5 * nx, y_wall + 0.5 * L
+    cx, cy = 0.5 * nx + x_offset, y_wall + 0.5 * L     # x_offset: off the mirror axis for parity runs (R16)
     disks = np.array([[cx, cy, R]])
     mask = rasterize_disks(nx, ny, disks)
     mask[0, :] = 1
