@@ -258,13 +258,12 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   };
   // own-position populations and phi of one march row; lower/upper: the row feeds c_y <= 0 / c_y >= 0
   auto issue_row = [&](unsigned u, int sn, int sp, int sc, bool lower, bool upper) {
-    unsigned cmin = 3u, cmax = 0u;   // classes: 0,1 fluid; 2 ghost; 3 bulk solid
+    unsigned cmin = 3u;   // least class of the lane's nodes: 0,1 fluid; 2 ghost; 3 bulk solid
 #pragma unroll
     for (int c = 0; c < NL; c++) {
       const unsigned cc = S.Cw[sc][lane][c] & 0xffu;
       cmin = min(cmin, cc);
     }
-    (void)cmax;
     const unsigned k = u + (unsigned)xa;
     if (cmin != 3u) cp_async_vec<VB>(sP0 + (unsigned)sp * P_STAGE, phi_in + k);
     if (cmin < 2u) {
