@@ -201,6 +201,12 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
     split = sim.step_timed(ks)
     t_collide = split["collide"] / ks * 1e-3          # s per launch of the dominant kernel
 
+    # ---- ceiling of the layout: a plain sector copy over the same state (no halos, no arithmetic) ----
+    try:
+        t_copy = sim.layout_copy_timed(20) * 1e-3
+    except Exception:
+        t_copy = None
+
     # ---- e2e through the C ABI with host buffers ----
     barrier()
     t0 = time.perf_counter()
@@ -227,7 +233,11 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
         roofline={"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                   "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_FUSED: "k_fused_step", binding.SCHEDULE_WARP: "k_fused_warp"}.get(schedule, "k_fused_pair"),
                   "bytes_per_launch": bytes_layout, "values_per_update": values,
-                  "kernel_ms": t_collide * 1e3, "kernel_share_of_step": split["collide"] / max(sum(split.values()), 1e-30),
+                  "kernel_ms": t_collide * 1e3,
+                  "layout_copy": None if t_copy is None else {
+                      "what": "plain copy of every 32-byte sector of the 9 N planes and phi that holds a fluid node "
+                              "(lbm_layout_copy_timed): what a pure streaming pass over this SoA-with-holes layout costs",
+                      "ms": t_copy * 1e3, "frac": bytes_layout / t_copy / 1e9 / peak, "kernel_over_copy": t_collide / t_copy}, "kernel_share_of_step": split["collide"] / max(sum(split.values()), 1e-30),
                   "canonical": {"bytes_per_update": 36 * rs + 1, "achieved": bytes_canon / t_collide / 1e9,
                                 "frac": bytes_canon / t_collide / 1e9 / peak,
                                 "note": "same time, counted as if all 18 N_i + 18 B_i moved (SURVEY 8(d) canonical)"}},

@@ -163,6 +163,14 @@ int lbm_node_update_batch(const lbm_params* prm, int64_t count, const double* N,
  * throughput and this call for the per-kernel split. */
 int lbm_step_timed(lbm_ctx* ctx, int64_t n, double ms[3]);
 
+/* Measurement helper: the ceiling of the state layout.  Runs `iters` passes of a plain copy kernel
+ * over the context's own arrays (every 32-byte sector of the 9 population planes and of phi that holds
+ * a fluid node is read and written once; no halos, no arithmetic; destination is scratch memory, the
+ * state is not disturbed) and returns the mean device time of one pass in milliseconds.  bench.py
+ * reports it beside the roofline fraction: it is what a pure streaming pass over this layout costs.
+ * LBM_EINVAL if nx*ny is not a whole number of sectors. */
+int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass);
+
 /* Device-timing helper: per-kernel-kind accumulated launch counts since the last reset;
  * counts[0] = collide(+stream), [1] = phi-sum, [2] = ghost, [3] = other. */
 int lbm_launch_counts(lbm_ctx* ctx, int64_t counts[4], int32_t reset);

@@ -24,7 +24,7 @@ FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
 EXPORTS = ("lbm_plan", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
            "lbm_get_populations", "lbm_keep_B", "lbm_sample_populations", "lbm_get_classification",
-           "lbm_diag", "lbm_node_update_batch", "lbm_step_timed", "lbm_launch_counts", "lbm_last_error", "lbm_version",
+           "lbm_diag", "lbm_node_update_batch", "lbm_step_timed", "lbm_layout_copy_timed", "lbm_launch_counts", "lbm_last_error", "lbm_version",
            "lbm_destroy")
 
 
@@ -107,6 +107,7 @@ def load_library() -> C.CDLL:
         L.lbm_step.argtypes = [vp, i64]
         L.lbm_sync.argtypes = [vp]
         L.lbm_step_timed.argtypes = [vp, i64, vp]
+        L.lbm_layout_copy_timed.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
         L.lbm_get.argtypes = [vp] * 6
         L.lbm_get_populations.argtypes = [vp, vp, vp]
         L.lbm_keep_B.argtypes = [vp, C.c_int32]
@@ -212,6 +213,12 @@ class LBM:
         ms = np.zeros(3)
         _check(load_library().lbm_step_timed(self._h, int(n), ms.ctypes.data), self._h)
         return dict(collide=float(ms[0]), phi_sum=float(ms[1]), ghost=float(ms[2]))
+
+    def layout_copy_timed(self, iters: int = 20) -> float:
+        """ms of one pass of the plain sector copy over this context's state (the layout's ceiling)."""
+        ms = C.c_double()
+        _check(load_library().lbm_layout_copy_timed(self._h, int(iters), C.byref(ms)), self._h)
+        return float(ms.value)
 
     def sync(self):
         _check(load_library().lbm_sync(self._h), self._h)

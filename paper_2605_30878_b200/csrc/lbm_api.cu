@@ -686,6 +686,36 @@ int lbm_diag(lbm_ctx* ctx, double out[8]) {
   return LBM_OK;
 }
 
+int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass) {
+  if (!ctx || iters < 1 || !ms_per_pass) return fail(ctx, LBM_EINVAL, "bad argument");
+  const size_t rs = ctx->is32 ? 4 : 8, nps = 32 / rs;
+  if (ctx->n % nps != 0 || ctx->Cd.ps % nps != 0) return fail(ctx, LBM_EINVAL, "nx*ny is not a whole number of 32-byte sectors");
+  const size_t nsec = ctx->n / nps, psec = ctx->Cd.ps / nps;
+  const float4* src = (const float4*)ctx->N[ctx->cur];
+  float4* dst = (float4*)ctx->N[ctx->cur ^ 1];          // scratch: the next step overwrites it
+  const float4* psrc = (const float4*)ctx->phi[ctx->pcur];
+  float4* pdst = (float4*)ctx->stage;                    // scratch (phi[pcur ^ 1] holds the previous ghost values)
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0));
+  CK(cudaEventCreate(&e1));
+  const int blocks = 148 * 32;
+  for (int it = 0; it < iters + 2; it++) {
+    if (it == 2) cudaEventRecord(e0, ctx->st);
+    if (ctx->is32) k_copy_sectors<8><<<blocks, 256, 0, ctx->st>>>(ctx->cl16, src, dst, psrc, pdst, nsec, psec);
+    else k_copy_sectors<4><<<blocks, 256, 0, ctx->st>>>(ctx->cl16, src, dst, psrc, pdst, nsec, psec);
+    ctx->launches[3]++;
+  }
+  cudaEventRecord(e1, ctx->st);
+  CK(cudaEventSynchronize(e1));
+  float ms = 0.f;
+  CK(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  CK(cudaGetLastError());
+  *ms_per_pass = (double)ms / iters;
+  return LBM_OK;
+}
+
 int lbm_launch_counts(lbm_ctx* ctx, int64_t counts[4], int32_t reset) {
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   if (counts) for (int k = 0; k < 4; k++) counts[k] = ctx->launches[k];

@@ -631,6 +631,34 @@ __global__ void __launch_bounds__(1024) k_diag_final(const DiagVec* __restrict__
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Measurement helper (lbm_layout_copy_timed): the ceiling of the SoA-with-holes layout.  One thread
+// per 32-byte sector of a population plane; a sector that holds a fluid node is copied whole, for
+// all 9 planes and phi.  No halos, no arithmetic: what a pure streaming pass over the state costs.
+// NPS = nodes per sector (8 in fp32, 4 in fp64).
+// ------------------------------------------------------------------------------------------
+template <int NPS>
+__global__ void __launch_bounds__(256) k_copy_sectors(const uint16_t* __restrict__ cl16, const float4* __restrict__ src,
+                                                      float4* __restrict__ dst, const float4* __restrict__ phi_src,
+                                                      float4* __restrict__ phi_dst, size_t nsec, size_t plane_sec) {
+  for (size_t k = (size_t)blockIdx.x * 256 + threadIdx.x; k < nsec; k += (size_t)gridDim.x * 256) {
+    bool any = false;
+    const unsigned* w = reinterpret_cast<const unsigned*>(cl16) + k * (NPS / 2);
+#pragma unroll
+    for (int t = 0; t < NPS / 2; t++) any |= ((w[t] & 0xffu) < 2u) || (((w[t] >> 16) & 0xffu) < 2u);
+    if (any) {
+#pragma unroll
+      for (int q = 0; q < 9; q++) {
+        const float4 a = src[(q * plane_sec + k) * 2], b = src[(q * plane_sec + k) * 2 + 1];
+        dst[(q * plane_sec + k) * 2] = a;
+        dst[(q * plane_sec + k) * 2 + 1] = b;
+      }
+      phi_dst[2 * k] = phi_src[2 * k];
+      phi_dst[2 * k + 1] = phi_src[2 * k + 1];
+    }
+  }
+}
+
 // test hook: independent nodes
 template <typename R>
 __global__ void __launch_bounds__(128) k_node_batch(const Consts<R> C, long long count,

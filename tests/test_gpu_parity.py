@@ -482,3 +482,18 @@ def test_paper_particle_at_interface_eq13():
         print("particle full", theta, h, h_an, s.diag()["umax"])
         assert abs(h - h_an) < 0.12 * abs(h_an)
         s.close()
+
+
+def test_layout_copy_helper_leaves_the_state_alone():
+    w = wl.config5(seed=2, n=256)
+    g, _ = make_pair(w)
+    g.init(w.phi0); g.step(7)
+    a = g.get()
+    ms_copy = g.layout_copy_timed(3)
+    g.step(5)
+    h, _ = make_pair(w)
+    h.init(w.phi0); h.step(12)
+    b, c = g.get(), h.get()
+    assert ms_copy > 0
+    for k in a:
+        assert np.array_equal(b[k], c[k]), k            # same as a run without the helper, bit for bit
