@@ -56,10 +56,15 @@ enum {
   LBM_SCHEDULE_WARP = 3,      /* 2 launches/step like FUSED but barrier-free: one warp marches down a
                                  30-column strip, phi(t+1) is assembled in registers by warp
                                  shuffles, loads run ahead through a per-warp cp.async ring        */
-  LBM_SCHEDULE_PAIR = 4       /* like WARP, but every lane owns an aligned pair of nodes: each
+  LBM_SCHEDULE_PAIR = 4,      /* like WARP, but every lane owns an aligned pair of nodes: each
                                  population is fetched once, unshifted, as an 8/16-byte vector;
                                  propagation in x is a warp shuffle; fp32 arithmetic is packed
                                  (FFMA2).  Needs even nx, else FUSED is used                        */
+  LBM_SCHEDULE_PACK = 5       /* the PAIR kernel on pair-compacted population planes: a plane stores
+                                 only the node pairs that hold a fluid node, row after row, without
+                                 holes (addressed through a 1-bit-per-pair mask + prefix table).  The
+                                 dense planes are kept as a mirror that lbm_get / lbm_diag / ... refresh
+                                 on demand.  Needs even nx, else FUSED is used                      */
 };
 
 typedef struct lbm_ctx lbm_ctx;                 /* opaque; one simulation                         */

@@ -2,6 +2,7 @@
 // the launch schedule.  No CPU fallback: every compute call needs a CUDA device.
 #include <cuda_runtime.h>
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -65,6 +66,14 @@ struct lbm_ctx {
   int* corner_p;
   void* wgt_p;
   uint8_t* csolid_p;
+  // PACK schedule: pair-compacted population planes (dense N[cur] is a mirror, refreshed on demand)
+  int packed;
+  int dense_valid;
+  int ccur;
+  int nw;            // ptab words per row
+  size_t cps;        // compact plane stride in pairs
+  uint2* ptab;
+  void* Nc[2];
   int* blk_cnt;
   int* blk_off;
   int* scal;          // [0] ghost total, [1] geometry error flag
@@ -113,7 +122,7 @@ int validate(const lbm_params* P, const char** why) {
   if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
   if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
   if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
-  if (P->schedule < 0 || P->schedule > 4) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 5) { *why = "unknown schedule"; return LBM_EINVAL; }
   if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
   return LBM_OK;
 }
@@ -171,7 +180,17 @@ bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELIN
 // one layout function serves both sizing (base == nullptr) and carving; everything that does not
 // depend on the ghost count comes first, so a carve with ng = 0 and one with the real ng agree
 // on those arrays
-size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
+bool use_pack(const lbm_params* P) { return P->schedule == LBM_SCHEDULE_PACK && (P->nx % 2) == 0; }
+
+// number of aligned node pairs that hold a fluid node (PACK schedule); mask: host, non-zero = solid
+long long count_fluid_pairs(const lbm_params* P, const uint8_t* mask) {
+  long long c = 0;
+  const size_t n = (size_t)P->nx * P->ny;
+  for (size_t k = 0; k + 1 < n; k += 2) c += (!mask[k] || !mask[k + 1]) ? 1 : 0;
+  return c;
+}
+
+size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long long nfp) {
   const size_t n = (size_t)P->nx * P->ny;
   const size_t rs = P->precision == 32 ? 4 : 8;
   const size_t g = (size_t)(ng > 0 ? ng : 1);
@@ -207,11 +226,22 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng) {
   int* corner_p = A.take<int>(4 * g);
   char* wgt_p = A.take<char>(4 * g * rs);
   uint8_t* csolid_p = A.take<uint8_t>(g);
+  // PACK schedule (last, so that nothing above depends on the pair count)
+  uint2* ptab = nullptr;
+  char *Nc0 = nullptr, *Nc1 = nullptr;
+  const int nw = (P->nx / 2 + 31) / 32;
+  const size_t cps = (((size_t)(nfp > 0 ? nfp : 1) + 63) & ~(size_t)63) + 37 * 64;
+  if (use_pack(P)) {
+    ptab = A.take<uint2>((size_t)P->ny * nw);
+    Nc0 = A.take<char>(9 * cps * 2 * rs);
+    Nc1 = A.take<char>(9 * cps * 2 * rs);
+  }
   if (c && base) {
     c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
     c->cls = cls; c->links = links; c->cl16 = cl16; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
     c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid;
-    c->gidx_p = gidx_p; c->corner_p = corner_p; c->wgt_p = wgt_p; c->csolid_p = csolid_p; c->blk_cnt = blk_cnt;
+    c->gidx_p = gidx_p; c->corner_p = corner_p; c->wgt_p = wgt_p; c->csolid_p = csolid_p;
+    c->ptab = ptab; c->Nc[0] = Nc0; c->Nc[1] = Nc1; c->nw = nw; c->cps = cps; c->blk_cnt = blk_cnt;
     c->blk_off = blk_off; c->scal = scal; c->stage = stage; c->diag_out = diag_out;
     c->samp_idx = samp; c->samp_cap = samp_cap;
   }
@@ -288,7 +318,14 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     const R* pi = (const R*)c->phi[c->pcur];
     R* po = (R*)c->phi[c->pcur ^ 1];
     bool done = false;
-    if (c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
+    if (c->packed) {   // PACK: compact planes step compact -> compact; the dense mirror N[cur] goes stale
+      done = launch_fused_pack(C, c->cl16, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po, c->st, c->ptab,
+                               c->nw, (unsigned)(c->cps * 2 * sizeof(R)));
+      c->ccur ^= 1;
+      c->dense_valid = 0;
+      c->cur ^= 1;     // undone below: the dense buffer index does not move
+    }
+    if (!done && c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
     if (!done && c->sched == LBM_SCHEDULE_WARP) done = launch_fused_warp<R>(C, c->cl16, Ns, Nd, Bd, pi, po, c->st) == 0;
     if (!done) launch_fused_step<R>(C, c->cls, c->links, Ns, Nd, Bd, pi, po, c->st);
     c->cur ^= 1;
@@ -310,6 +347,21 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     tm->ms[0] += a; tm->ms[1] += b; tm->ms[2] += g;
   }
   return LBM_OK;
+}
+
+// PACK schedule: refresh the dense mirror N[cur] from the compact planes before a dense reader runs
+void ensure_dense(lbm_ctx* c) {
+  if (!c->packed || c->dense_valid) return;
+  const long long np = (long long)c->P.ny * (c->P.nx / 2);
+  const unsigned nb = (unsigned)((np + 255) / 256);
+  if (c->is32)
+    k_pair_repack<float, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, c->Cf.ps, c->cps,
+                                                       (float*)c->N[c->cur], (float*)c->Nc[c->ccur]);
+  else
+    k_pair_repack<double, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, c->Cd.ps, c->cps,
+                                                        (double*)c->N[c->cur], (double*)c->Nc[c->ccur]);
+  c->launches[3]++;
+  c->dense_valid = 1;
 }
 
 const void* B_planes(const lbm_ctx* c) { return c->fused ? c->B[0] : c->B[c->cur]; }
@@ -346,7 +398,7 @@ int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_
   cudaFree(d_tot);
   if (e != cudaSuccess) return cuda_fail(nullptr, e, "lbm_plan");
   if (n_ghost) *n_ghost = (int64_t)tot;
-  if (workspace_bytes) *workspace_bytes = layout(nullptr, nullptr, prm, (long long)tot);
+  if (workspace_bytes) *workspace_bytes = layout(nullptr, nullptr, prm, (long long)tot, use_pack(prm) ? count_fluid_pairs(prm, mask) : 0);
   return LBM_OK;
 }
 
@@ -363,7 +415,8 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   if (!d_workspace || ((uintptr_t)d_workspace & 255)) return fail(nullptr, LBM_EINVAL, "workspace null or not 256-byte aligned");
   const size_t n = (size_t)prm->nx * prm->ny;
   // the disk list and the mask upload need room before the ghost count is known
-  const size_t min_ws = layout(nullptr, nullptr, prm, 0);
+  const long long nfp = use_pack(prm) ? count_fluid_pairs(prm, mask) : 0;
+  const size_t min_ws = layout(nullptr, nullptr, prm, 0, nfp);
   if (workspace_bytes < min_ws) return fail(nullptr, LBM_ENOMEM, "workspace too small");
 
 #ifdef LBM_L2_FETCH
@@ -381,7 +434,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   c->st = (cudaStream_t)cuda_stream;
   c->Cd = make_consts<double>(*prm);
   c->Cf = make_consts<float>(*prm);
-  layout(c, (char*)d_workspace, prm, 0);   // provisional carve: cls/links/blk arrays do not depend on ng
+  layout(c, (char*)d_workspace, prm, 0, nfp);   // provisional carve: cls/links/blk arrays do not depend on ng
 
 #define CKC(call)                                                              \
   do {                                                                         \
@@ -401,12 +454,12 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   CKC(cudaMemcpyAsync(&ng, c->scal, sizeof(int), cudaMemcpyDeviceToHost, c->st));
   CKC(cudaStreamSynchronize(c->st));
   c->ng = ng;
-  const size_t need = layout(nullptr, nullptr, prm, ng);
+  const size_t need = layout(nullptr, nullptr, prm, ng, nfp);
   if (workspace_bytes < need) {
     delete c;
     return fail(nullptr, LBM_ENOMEM, "workspace too small for the ghost list (size it with lbm_plan)");
   }
-  layout(c, (char*)d_workspace, prm, ng);   // ghost arrays now have their real extent
+  layout(c, (char*)d_workspace, prm, ng, nfp);   // ghost arrays now have their real extent
 
   // (2) index-sorted ghost list and per-ghost geometry
   if (ng > 0) {
@@ -489,6 +542,30 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
       if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "ghost processing order"); }
     }
   }
+  if (use_pack(prm)) {   // PACK schedule: pair mask words and their compact base indices
+    const long long nwords = (long long)prm->ny * c->nw;
+    unsigned* pmask = nullptr;
+    void* tmp = nullptr;
+    size_t tmp_bytes = 0;
+    cudaError_t e = cudaMalloc(&pmask, 3 * sizeof(int) * (size_t)nwords + 16);
+    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(pair table)"); }
+    int* pcount = reinterpret_cast<int*>(pmask + nwords);
+    int* pbase = pcount + nwords;
+    const unsigned nb = (unsigned)((nwords + 255) / 256);
+    k_pair_mask<<<nb, 256, 0, c->st>>>(c->cls, prm->nx, prm->ny, c->nw, pmask, pcount);
+    e = cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, pcount, pbase, (int)nwords, c->st);
+    if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 1);
+    if (e == cudaSuccess) e = cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, pcount, pbase, (int)nwords, c->st);
+    if (e == cudaSuccess) {
+      k_pair_tab<<<nb, 256, 0, c->st>>>(pmask, pbase, nwords, c->ptab);
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    cudaFree(tmp);
+    cudaFree(pmask);
+    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "pair table"); }
+    c->packed = 1;
+  }
   CKC(cudaStreamSynchronize(c->st));
 #undef CKC
   *out = c;
@@ -518,6 +595,18 @@ int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
                                              (double*)Bp, (double*)ctx->phi[0], (double*)ctx->phi[1]);
   ctx->launches[3]++;
   ctx->B_valid = 1;
+  if (ctx->packed) {   // PACK: the compact planes start as a copy of the dense initial state
+    const long long np = (long long)ctx->P.ny * (ctx->P.nx / 2);
+    const unsigned nb = (unsigned)((np + 255) / 256);
+    if (ctx->is32)
+      k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, ctx->Cf.ps, ctx->cps,
+                                                          (float*)ctx->N[0], (float*)ctx->Nc[0]);
+    else
+      k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, ctx->Cd.ps, ctx->cps,
+                                                           (double*)ctx->N[0], (double*)ctx->Nc[0]);
+    ctx->ccur = 0;
+    ctx->dense_valid = 1;
+  }
   if (ctx->is32) launch_ghost<float>(ctx); else launch_ghost<double>(ctx);
   CK(cudaGetLastError());
   CK(cudaStreamSynchronize(ctx->st));
@@ -563,6 +652,7 @@ int lbm_keep_B(lbm_ctx* ctx, int32_t on) {
 }
 
 int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, double* p) {
+  if (ctx) ensure_dense(ctx);
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   const size_t n = ctx->n;
   double* s = ctx->stage;
@@ -586,6 +676,7 @@ int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, doub
 }
 
 int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
+  if (ctx) ensure_dense(ctx);
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   if (B && !ctx->B_valid)
     return fail(ctx, LBM_EINVAL, "B is not stored under this schedule: call lbm_keep_B(ctx, 1) before lbm_step");
@@ -619,6 +710,7 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
 }
 
 int lbm_sample_populations(lbm_ctx* ctx, int64_t n_idx, const int64_t* idx, double* N, double* B) {
+  if (ctx) ensure_dense(ctx);
   if (!ctx || n_idx < 0 || (n_idx > 0 && !idx)) return fail(ctx, LBM_EINVAL, "bad argument");
   if (B && !ctx->B_valid)
     return fail(ctx, LBM_EINVAL, "B is not stored under this schedule: call lbm_keep_B(ctx, 1) before lbm_step");
@@ -666,6 +758,7 @@ int lbm_get_classification(lbm_ctx* ctx, uint8_t* cls, int32_t* n_ghost, int32_t
 }
 
 int lbm_diag(lbm_ctx* ctx, double out[8]) {
+  if (ctx) ensure_dense(ctx);
   if (!ctx || !out) return fail(ctx, LBM_EINVAL, "null argument");
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
@@ -687,6 +780,7 @@ int lbm_diag(lbm_ctx* ctx, double out[8]) {
 }
 
 int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass) {
+  if (ctx) ensure_dense(ctx);
   if (!ctx || iters < 1 || !ms_per_pass) return fail(ctx, LBM_EINVAL, "bad argument");
   const size_t rs = ctx->is32 ? 4 : 8, nps = 32 / rs;
   if (ctx->n % nps != 0 || ctx->Cd.ps % nps != 0) return fail(ctx, LBM_EINVAL, "nx*ny is not a whole number of 32-byte sectors");

@@ -171,7 +171,7 @@ __device__ __forceinline__ void cp_async_vec(unsigned saddr, const void* gptr) {
 
 // shared-memory ring of one warp: row stages hold the own-position populations and phi of the strip;
 // class stages the packed class words (NL 16-bit words per lane)
-template <typename V, int DP>
+template <typename V, int DP, bool PACKED>
 struct PairRing {
   static constexpr int NL = LaneOf<V>::NL;
   static constexpr int NS = DP + 2;        // population rows i-1 (until refilled) .. i+1+DP
@@ -180,6 +180,7 @@ struct PairRing {
   V N[NS][9][32];
   V P[PS][32];
   unsigned short Cw[CS][32][NL];
+  uint2 Tb[PACKED ? CS : 1][32];           // PACK schedule: {pair mask word, compact index of its first pair}
 };
 
 // collide the NL nodes of a lane (fl[c]: node c is fluid).  All nodes always go through the
@@ -207,15 +208,19 @@ __device__ __forceinline__ void collide_lane(const Consts<typename LaneOf<V>::R>
   }
 }
 
-template <typename V, int DP, int WARPS, int MINB, bool WRITE_B>
+// PACKED: the population planes are pair-compacted (PACK schedule, see k_pair_mask): Nsrc / Ndst hold only
+// the pairs with a fluid node, plane stride cpsB bytes, addressed through ptab (nw words per row).
+template <typename V, int DP, int WARPS, int MINB, bool WRITE_B, bool PACKED>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
     k_fused_pair(const Consts<typename LaneOf<V>::R> C, const uint16_t* __restrict__ cl16,
                  const typename LaneOf<V>::R* __restrict__ Nsrc, typename LaneOf<V>::R* __restrict__ Ndst,
                  typename LaneOf<V>::R* __restrict__ Bdst, const typename LaneOf<V>::R* __restrict__ phi_in,
-                 typename LaneOf<V>::R* __restrict__ phi_out, int TY) {
+                 typename LaneOf<V>::R* __restrict__ phi_out, int TY, const uint2* __restrict__ ptab, int nw,
+                 unsigned cpsB) {
   using L = LaneOf<V>;
   using R = typename L::R;
-  using Ring = PairRing<V, DP>;
+  using Ring = PairRing<V, DP, PACKED>;
+  static_assert(!PACKED || L::NL == 2, "the PACK schedule compacts node pairs");
   constexpr int NL = L::NL;
   constexpr int OUTC = 30 * NL;            // output columns of a strip
   constexpr unsigned FULL = 0xffffffffu;
@@ -224,13 +229,15 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Ring& S = reinterpret_cast<Ring*>(smem_raw)[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
-  const unsigned sN0 = (unsigned)__cvta_generic_to_shared(&S.N[0][0][lane]);
+  const unsigned sN0 = (unsigned)__cvta_generic_to_shared(&S.N[0][0][PACKED ? 0 : lane]);
   const unsigned sP0 = (unsigned)__cvta_generic_to_shared(&S.P[0][lane]);
   const unsigned sC0 = (unsigned)__cvta_generic_to_shared(&S.Cw[0][lane][0]);
+  const unsigned sT0 = (unsigned)__cvta_generic_to_shared(&S.Tb[0][lane]);
   constexpr unsigned N_STAGE = 9 * 32 * VB, N_PLANE = 32 * VB, P_STAGE = 32 * VB, C_STAGE = 32 * NL * 2;
 
   const int nx = C.nx, ny = C.ny;   // nx is a multiple of NL (checked by the launcher)
-  const unsigned psB = (unsigned)C.ps * (unsigned)sizeof(R);   // plane stride in bytes (< 2^32: lbm_create)
+  const unsigned psB = PACKED ? cpsB : (unsigned)C.ps * (unsigned)sizeof(R);   // plane stride in bytes (< 2^32: lbm_create)
+  const unsigned psBd = (unsigned)C.ps * (unsigned)sizeof(R);                  // dense stride (B planes of lbm_keep_B)
   const int g = blockIdx.x * WARPS + (threadIdx.x >> 5);
   if (OUTC * g >= nx) return;                            // whole warp; the kernel has no block barrier
   const int xend = min(OUTC * g + OUTC, nx);             // one past the last output column (multiple of NL)
@@ -238,6 +245,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   const bool col_out = lane >= 1 && lane <= 30 && lxa < xend;
   int xa = lxa % nx;                                     // every lane is a valid periodic group
   if (xa < 0) xa += nx;
+  const int pword = (xa / 2) >> 5;                       // PACK: word and bit of the lane's pair in ptab
+  const unsigned pbit = (unsigned)(xa / 2) & 31u, plt = (1u << pbit) - 1u;
   // lanes whose groups share a 32-byte sector of a population plane (rows keep the sector phase only
   // if the row pitch is a multiple of 32 bytes); a sector that holds any fluid node is stored whole
   // (zeros on its solid nodes), so that HBM never has to read-modify-write a partial sector
@@ -253,8 +262,9 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   };
   auto inc = [](int v, int mod) { return v + 1 == mod ? 0 : v + 1; };
   // ---- asynchronous fetches (slots and row offsets are passed in: no modulo in the march) ----
-  auto issue_cls = [&](unsigned u, int sc) {   // the NL class words of the lane (one aligned word)
-    cp_async_vec<NL * 2>(sC0 + (unsigned)sc * C_STAGE, cl16 + (u + (unsigned)xa));
+  auto issue_cls = [&](int r, int sc) {   // the NL class words of the lane in grid row r (one aligned word)
+    cp_async_vec<NL * 2>(sC0 + (unsigned)sc * C_STAGE, cl16 + ((unsigned)r * (unsigned)nx + (unsigned)xa));
+    if (PACKED) cp_async_vec<8>(sT0 + (unsigned)sc * 256u, ptab + ((size_t)r * nw + pword));
   };
   // own-position populations and phi of one march row; lower/upper: the row feeds c_y <= 0 / c_y >= 0
   auto issue_row = [&](unsigned u, int sn, int sp, int sc, bool lower, bool upper) {
@@ -267,8 +277,15 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     const unsigned k = u + (unsigned)xa;
     if (cmin != 3u) cp_async_vec<VB>(sP0 + (unsigned)sp * P_STAGE, phi_in + k);
     if (cmin < 2u) {
-      const unsigned d = sN0 + (unsigned)sn * N_STAGE;
-      const char* src = reinterpret_cast<const char*>(Nsrc + k);   // plane q is src + q * psB
+      unsigned ke = k;                                             // element offset of the group in a plane
+      unsigned d = sN0 + (unsigned)sn * N_STAGE;
+      if (PACKED) {
+        const uint2 tb = S.Tb[sc][lane];
+        const unsigned ci = tb.y + (unsigned)__popc(tb.x & plt);
+        ke = ci * 2u;
+        d += (unsigned)lane * VB;   // entry = lane (an entry aligned to the compact index was tried: no gain)
+      }
+      const char* src = reinterpret_cast<const char*>(Nsrc + ke);   // plane q is src + q * psB
       if (lower && upper) {
         cp_async_vec<VB>(d + 0 * N_PLANE, src);
         cp_async_vec<VB>(d + 1 * N_PLANE, src + (size_t)psB * 1u);
@@ -298,7 +315,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     for (int s = 0; s < PS; s++) S.P[s][lane] = zero;
   }
   for (int m = -1; m <= 2 * DP; m++)
-    if (m <= last + 1) issue_cls((unsigned)wrap_row(m) * (unsigned)nx, (m + 1) % CS);
+    if (m <= last + 1) issue_cls(wrap_row(m), (m + 1) % CS);
   cp_async_commit();
   cp_async_wait<0>();
   for (int m = -1; m <= DP; m++) {
@@ -322,16 +339,17 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   for (int i = 0; i <= last; i++) {
     cp_async_wait<DP - 1>();   // row i+1 and the class words of row i+1+DP have landed
     // operands that live in the slot about to be refilled: planes 2,5,6 of row i-1
-    const V Bp0 = S.N[sN_a][2][lane], Bp1 = S.N[sN_a][5][lane], Bp2 = S.N[sN_a][6][lane];
+    const int lm = lane, lc = lane, ln = lane;   // ring entries of the lane's group in rows i-1, i, i+1
+    const V Bp0 = S.N[sN_a][2][lm], Bp1 = S.N[sN_a][5][lm], Bp2 = S.N[sN_a][6][lm];
     const V pS = S.P[sP_a][lane];
     // ---- issue: populations and phi of row i+1+DP, class words of row i+1+2DP ----
     if (i + 1 + DP <= last + 1) issue_row((unsigned)rf * (unsigned)nx, sN_a, sP_f, sC_f, true, i + 1 + DP <= last);
-    if (i + 1 + 2 * DP <= last + 1) issue_cls((unsigned)rc * (unsigned)nx, sC_n);
+    if (i + 1 + 2 * DP <= last + 1) issue_cls(rc, sC_n);
     cp_async_commit();
 
     // ---- on-chip operands of march row i ----
-    const V A0 = S.N[sN_b][0][lane], A1 = S.N[sN_b][1][lane], A3 = S.N[sN_b][3][lane];
-    const V Cn0 = S.N[sN_c][4][lane], Cn1 = S.N[sN_c][7][lane], Cn2 = S.N[sN_c][8][lane];
+    const V A0 = S.N[sN_b][0][lc], A1 = S.N[sN_b][1][lc], A3 = S.N[sN_b][3][lc];
+    const V Cn0 = S.N[sN_c][4][ln], Cn1 = S.N[sN_c][7][ln], Cn2 = S.N[sN_c][8][ln];
     const V pC = S.P[sP_b][lane], pN = S.P[sP_c][lane];
 
     bool fl[NL];
@@ -353,8 +371,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     nn[2] = Bp0; nn[5] = from_left(Bp1);  nn[6] = from_right(Bp2);
     nn[4] = Cn0; nn[7] = from_right(Cn1); nn[8] = from_left(Cn2);
     if (any_link) {   // warp-uniform; half-way bounce-back (R12): own opposite population, same row
-      const V own[9] = {A0, A1, S.N[sN_b][2][lane], A3, S.N[sN_b][4][lane], S.N[sN_b][5][lane],
-                        S.N[sN_b][6][lane], S.N[sN_b][7][lane], S.N[sN_b][8][lane]};   // plane q at (x, i)
+      const V own[9] = {A0, A1, S.N[sN_b][2][lc], A3, S.N[sN_b][4][lc], S.N[sN_b][5][lc],
+                        S.N[sN_b][6][lc], S.N[sN_b][7][lc], S.N[sN_b][8][lc]};   // plane q at (x, i)
 #pragma unroll
       for (int q = 1; q < 9; q++) {
         R a[NL], o[NL];
@@ -367,7 +385,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       }
     }
     const unsigned fmask = __ballot_sync(FULL, col_out && any_fl);
-    const bool st = col_out && i >= 1 && i <= rows && (fmask & gmask) != 0u;   // my sector holds a fluid node
+    // dense planes: my sector holds a fluid node; compact planes have no holes: my pair holds one
+    const bool st = col_out && i >= 1 && i <= rows && (PACKED ? any_fl : (fmask & gmask) != 0u);
     // phi stencil (R8): west / east neighbours of the three rows (shuffles: all lanes take part)
     const V pCw = from_left(pC), pCe = from_right(pC), pNw = from_left(pN), pNe = from_right(pN);
     const V pSw = from_left(pS), pSe = from_right(pS);
@@ -379,13 +398,18 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       V ns[9];
       collide_lane<V>(C, nn, ph, fl, all_fl, ns, bs);
       if (st) {
-        char* dst = reinterpret_cast<char*>(Ndst + kout);
+        unsigned ko = kout;
+        if (PACKED) {
+          const uint2 tb = S.Tb[sC_i][lane];
+          ko = (tb.y + (unsigned)__popc(tb.x & plt)) * 2u;
+        }
+        char* dst = reinterpret_cast<char*>(Ndst + ko);
 #pragma unroll
         for (int q = 0; q < 9; q++) store_vec<V>(dst + (size_t)psB * (unsigned)q, ns[q]);
         if (WRITE_B) {
           char* dstB = reinterpret_cast<char*>(Bdst + kout);
 #pragma unroll
-          for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dstB + (size_t)psB * (unsigned)q) = bs[q];
+          for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dstB + (size_t)psBd * (unsigned)q) = bs[q];
         }
       }
       if (lk_any) {   // link q hands the node its own B_opp(q)* back
@@ -439,10 +463,11 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   cp_async_wait<0>();
 }
 
-template <typename V, int DP, int MINB>
+template <typename V, int DP, int MINB, bool PACKED>
 bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* cl16,
                        const typename LaneOf<V>::R* Nsrc, typename LaneOf<V>::R* Ndst, typename LaneOf<V>::R* Bdst,
-                       const typename LaneOf<V>::R* phi_in, typename LaneOf<V>::R* phi_out, cudaStream_t st) {
+                       const typename LaneOf<V>::R* phi_in, typename LaneOf<V>::R* phi_out, cudaStream_t st,
+                       const uint2* ptab = nullptr, int nw = 0, unsigned cpsB = 0) {
   constexpr int WARPS = LBM_PAIR_WARPS;
   constexpr int OUTC = 30 * LaneOf<V>::NL;
   const int nwx = (C.nx + OUTC - 1) / OUTC;
@@ -451,14 +476,14 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   int TY = LBM_PAIR_TY;
   while (TY > 8 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 8) TY >>= 1;
   const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
-  const size_t smem = sizeof(PairRing<V, DP>) * WARPS;
-  auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true> : k_fused_pair<V, DP, WARPS, MINB, false>;
+  const size_t smem = sizeof(PairRing<V, DP, PACKED>) * WARPS;
+  auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true, PACKED> : k_fused_pair<V, DP, WARPS, MINB, false, PACKED>;
   static bool attr_set[2] = {false, false};
   if (!attr_set[Bdst ? 1 : 0]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
     attr_set[Bdst ? 1 : 0] = true;
   }
-  kern<<<grid, 32 * WARPS, smem, st>>>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, TY);
+  kern<<<grid, 32 * WARPS, smem, st>>>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, TY, ptab, nw, cpsB);
   return true;
 }
 
@@ -466,14 +491,26 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
 inline bool launch_fused_pair(const Consts<double>& C, const uint16_t* cl16, const double* Nsrc, double* Ndst,
                               double* Bdst, const double* phi_in, double* phi_out, cudaStream_t st) {
   if (C.nx & 1) return false;
-  return launch_fused_lane<D2, LBM_PAIR_DP64, LBM_PAIR_MINB64>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
+  return launch_fused_lane<D2, LBM_PAIR_DP64, LBM_PAIR_MINB64, false>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
 }
 inline bool launch_fused_pair(const Consts<float>& C, const uint16_t* cl16, const float* Nsrc, float* Ndst,
                               float* Bdst, const float* phi_in, float* phi_out, cudaStream_t st) {
   if (C.nx & 1) return false;
   if (LBM_PAIR_QUAD && (C.nx & 3) == 0)
-    return launch_fused_lane<Q4, LBM_PAIR_DP32, LBM_PAIR_MINBQ>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
-  return launch_fused_lane<F2, LBM_PAIR_DP32, LBM_PAIR_MINB32>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
+    return launch_fused_lane<Q4, LBM_PAIR_DP32, LBM_PAIR_MINBQ, false>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
+  return launch_fused_lane<F2, LBM_PAIR_DP32, LBM_PAIR_MINB32, false>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
+}
+
+// PACK schedule: the same kernel on pair-compacted planes (Nsrc / Ndst are the compact buffers)
+inline bool launch_fused_pack(const Consts<double>& C, const uint16_t* cl16, const double* Nsrc, double* Ndst,
+                              double* Bdst, const double* phi_in, double* phi_out, cudaStream_t st,
+                              const uint2* ptab, int nw, unsigned cpsB) {
+  return launch_fused_lane<D2, LBM_PAIR_DP64, LBM_PAIR_MINB64, true>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st, ptab, nw, cpsB);
+}
+inline bool launch_fused_pack(const Consts<float>& C, const uint16_t* cl16, const float* Nsrc, float* Ndst,
+                              float* Bdst, const float* phi_in, float* phi_out, cudaStream_t st,
+                              const uint2* ptab, int nw, unsigned cpsB) {
+  return launch_fused_lane<F2, LBM_PAIR_DP32, LBM_PAIR_MINB32, true>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st, ptab, nw, cpsB);
 }
 
 }  // namespace lbm

@@ -13,9 +13,9 @@ from paper_2605_30878_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-BASELINE, FUSED, WARP, PAIR = 1, 2, 3, 4
+BASELINE, FUSED, WARP, PAIR, PACK = 1, 2, 3, 4, 5
 SCHEDULES = [pytest.param(BASELINE, id="baseline"), pytest.param(FUSED, id="fused"), pytest.param(WARP, id="warp"),
-             pytest.param(PAIR, id="pair")]
+             pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack")]
 
 
 # ---- local update of single nodes ---------------------------------------------------------------
@@ -281,7 +281,8 @@ def test_config3_density_ratio_1000_short():
         assert err["rho"] <= tol * scale["rho"]          # rho = rho_g + 999 phi: relative to field scale
 
 
-@pytest.mark.parametrize("sched", [pytest.param(FUSED, id="fused"), pytest.param(WARP, id="warp"), pytest.param(PAIR, id="pair")])
+@pytest.mark.parametrize("sched", [pytest.param(FUSED, id="fused"), pytest.param(WARP, id="warp"), pytest.param(PAIR, id="pair"),
+                                   pytest.param(PACK, id="pack")])
 def test_schedules_agree_and_get_is_idempotent(sched):
     w = wl.config5(seed=3, n=256)
     a, _ = make_pair(w, schedule=BASELINE)
