@@ -186,7 +186,12 @@ bool use_pack(const lbm_params* P) { return P->schedule == LBM_SCHEDULE_PACK && 
 long long count_fluid_pairs(const lbm_params* P, const uint8_t* mask) {
   long long c = 0;
   const size_t n = (size_t)P->nx * P->ny;
-  for (size_t k = 0; k + 1 < n; k += 2) c += (!mask[k] || !mask[k + 1]) ? 1 : 0;
+  const size_t G = (size_t)pack_group(P->precision == 32 ? 4 : 8, P->nx);
+  for (size_t k = 0; k + G <= n; k += G) {
+    bool any = false;
+    for (size_t t = 0; t < G; t++) any |= !mask[k + t];
+    c += any ? 1 : 0;
+  }
   return c;
 }
 
@@ -229,12 +234,13 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
   // PACK schedule (last, so that nothing above depends on the pair count)
   uint2* ptab = nullptr;
   char *Nc0 = nullptr, *Nc1 = nullptr;
-  const int nw = (P->nx / 2 + 31) / 32;
+  const int G = pack_group(P->precision == 32 ? 4 : 8, P->nx);
+  const int nw = (P->nx / G + 31) / 32;
   const size_t cps = (((size_t)(nfp > 0 ? nfp : 1) + 63) & ~(size_t)63) + 37 * 64;
   if (use_pack(P)) {
     ptab = A.take<uint2>((size_t)P->ny * nw);
-    Nc0 = A.take<char>(9 * cps * 2 * rs);
-    Nc1 = A.take<char>(9 * cps * 2 * rs);
+    Nc0 = A.take<char>(9 * cps * G * rs);
+    Nc1 = A.take<char>(9 * cps * G * rs);
   }
   if (c && base) {
     c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
@@ -320,7 +326,7 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     bool done = false;
     if (c->packed) {   // PACK: compact planes step compact -> compact; the dense mirror N[cur] goes stale
       done = launch_fused_pack(C, c->cl16, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po, c->st, c->ptab,
-                               c->nw, (unsigned)(c->cps * 2 * sizeof(R)));
+                               c->nw, (unsigned)(c->cps * pack_group((int)sizeof(R), c->P.nx) * sizeof(R)));
       c->ccur ^= 1;
       c->dense_valid = 0;
       c->cur ^= 1;     // undone below: the dense buffer index does not move
@@ -352,13 +358,14 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
 // PACK schedule: refresh the dense mirror N[cur] from the compact planes before a dense reader runs
 void ensure_dense(lbm_ctx* c) {
   if (!c->packed || c->dense_valid) return;
-  const long long np = (long long)c->P.ny * (c->P.nx / 2);
+  const int G = pack_group(c->is32 ? 4 : 8, c->P.nx);
+  const long long np = (long long)c->P.ny * (c->P.nx / G);
   const unsigned nb = (unsigned)((np + 255) / 256);
   if (c->is32)
-    k_pair_repack<float, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, c->Cf.ps, c->cps,
+    k_pair_repack<float, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, G, c->Cf.ps, c->cps,
                                                        (float*)c->N[c->cur], (float*)c->Nc[c->ccur]);
   else
-    k_pair_repack<double, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, c->Cd.ps, c->cps,
+    k_pair_repack<double, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, G, c->Cd.ps, c->cps,
                                                         (double*)c->N[c->cur], (double*)c->Nc[c->ccur]);
   c->launches[3]++;
   c->dense_valid = 1;
@@ -552,7 +559,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     int* pcount = reinterpret_cast<int*>(pmask + nwords);
     int* pbase = pcount + nwords;
     const unsigned nb = (unsigned)((nwords + 255) / 256);
-    k_pair_mask<<<nb, 256, 0, c->st>>>(c->cls, prm->nx, prm->ny, c->nw, pmask, pcount);
+    k_pair_mask<<<nb, 256, 0, c->st>>>(c->cls, prm->nx, prm->ny, c->nw, pack_group(c->is32 ? 4 : 8, prm->nx), pmask, pcount);
     e = cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, pcount, pbase, (int)nwords, c->st);
     if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 1);
     if (e == cudaSuccess) e = cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, pcount, pbase, (int)nwords, c->st);
@@ -596,13 +603,14 @@ int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
   ctx->launches[3]++;
   ctx->B_valid = 1;
   if (ctx->packed) {   // PACK: the compact planes start as a copy of the dense initial state
-    const long long np = (long long)ctx->P.ny * (ctx->P.nx / 2);
+    const int G = pack_group(ctx->is32 ? 4 : 8, ctx->P.nx);
+    const long long np = (long long)ctx->P.ny * (ctx->P.nx / G);
     const unsigned nb = (unsigned)((np + 255) / 256);
     if (ctx->is32)
-      k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, ctx->Cf.ps, ctx->cps,
+      k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cf.ps, ctx->cps,
                                                           (float*)ctx->N[0], (float*)ctx->Nc[0]);
     else
-      k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, ctx->Cd.ps, ctx->cps,
+      k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cd.ps, ctx->cps,
                                                            (double*)ctx->N[0], (double*)ctx->Nc[0]);
     ctx->ccur = 0;
     ctx->dense_valid = 1;

@@ -660,22 +660,25 @@ __global__ void __launch_bounds__(256) k_copy_sectors(const uint16_t* __restrict
 }
 
 // ------------------------------------------------------------------------------------------
-// PACK schedule: pair-compacted population planes.  A plane stores only the aligned node pairs that
-// hold a fluid node, row after row, without holes.  ptab[r * nw + w] = {bit b set <=> pair 32 w + b of
-// row r holds a fluid node, compact index of the first pair of that word}; the compact index of pair
-// p of row r is ptab[..].y + popc(ptab[..].x & ((1 << (p & 31)) - 1)).
+// PACK schedule: group-compacted population planes.  A plane stores only the aligned groups of G
+// x-adjacent nodes (G = nodes per lane of the kernel: 2, or 4 for the fp32 quad variant) that hold a
+// fluid node, row after row, without holes.  ptab[r * nw + w] = {bit b set <=> group 32 w + b of row r
+// holds a fluid node, compact index of the first group of that word}; the compact index of group p of
+// row r is ptab[..].y + popc(ptab[..].x & ((1 << (p & 31)) - 1)).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_pair_mask(const uint8_t* __restrict__ cls, int nx, int ny, int nw,
+__global__ void __launch_bounds__(256) k_pair_mask(const uint8_t* __restrict__ cls, int nx, int ny, int nw, int G,
                                                    unsigned* __restrict__ pmask, int* __restrict__ pcount) {
   const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
   if (t >= (long long)ny * nw) return;
   const int r = (int)(t / nw), w = (int)(t % nw);
   unsigned m = 0;
   for (int b = 0; b < 32; b++) {
-    const int x = 2 * (32 * w + b);
+    const int x = G * (32 * w + b);
     if (x < nx) {
       const size_t k = (size_t)r * nx + x;
-      if (cls[k] < 2 || cls[k + 1] < 2) m |= 1u << b;
+      bool any = false;
+      for (int c = 0; c < G; c++) any |= cls[k + c] < 2;
+      if (any) m |= 1u << b;
     }
   }
   pmask[t] = m;
@@ -686,29 +689,25 @@ __global__ void __launch_bounds__(256) k_pair_tab(const unsigned* __restrict__ p
   const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
   if (t < nwords) ptab[t] = make_uint2(pmask[t], (unsigned)pbase[t]);
 }
-// dense (pop[q * ps + k]) <-> compact (popc[(q * cps + ci) * 2 + c]) copies of the 9 planes; TO_COMPACT
-// packs, else unpacks (the solid partner of a pair travels with it; other dense entries are untouched)
+// dense (pop[q * ps + k]) <-> compact (popc[(q * cps + ci) * G + c]) copies of the 9 planes; TO_COMPACT
+// packs, else unpacks (the solid nodes of a group travel with it; other dense entries are untouched)
 template <typename R, bool TO_COMPACT>
-__global__ void __launch_bounds__(256) k_pair_repack(const uint2* __restrict__ ptab, int nx, int ny, int nw, size_t ps,
-                                                     size_t cps, R* __restrict__ dense, R* __restrict__ compact) {
-  const long long t = (long long)blockIdx.x * 256 + threadIdx.x;   // one thread per pair
-  const int npr = nx / 2;
+__global__ void __launch_bounds__(256) k_pair_repack(const uint2* __restrict__ ptab, int nx, int ny, int nw, int G,
+                                                     size_t ps, size_t cps, R* __restrict__ dense,
+                                                     R* __restrict__ compact) {
+  const long long t = (long long)blockIdx.x * 256 + threadIdx.x;   // one thread per group
+  const int npr = nx / G;
   if (t >= (long long)ny * npr) return;
   const int r = (int)(t / npr), p = (int)(t % npr);
   const uint2 tb = ptab[(size_t)r * nw + (p >> 5)];
   if (!((tb.x >> (p & 31)) & 1u)) return;
   const size_t ci = (size_t)tb.y + (size_t)__popc(tb.x & ((1u << (p & 31)) - 1u));
-  const size_t k = (size_t)r * nx + 2 * (size_t)p;
-#pragma unroll
-  for (int q = 0; q < 9; q++) {
-    if (TO_COMPACT) {
-      compact[(q * cps + ci) * 2] = dense[q * ps + k];
-      compact[(q * cps + ci) * 2 + 1] = dense[q * ps + k + 1];
-    } else {
-      dense[q * ps + k] = compact[(q * cps + ci) * 2];
-      dense[q * ps + k + 1] = compact[(q * cps + ci) * 2 + 1];
+  const size_t k = (size_t)r * nx + (size_t)G * p;
+  for (int q = 0; q < 9; q++)
+    for (int c = 0; c < G; c++) {
+      if (TO_COMPACT) compact[(q * cps + ci) * G + c] = dense[q * ps + k + c];
+      else dense[q * ps + k + c] = compact[(q * cps + ci) * G + c];
     }
-  }
 }
 
 // test hook: independent nodes

@@ -52,6 +52,9 @@ namespace lbm {
 #ifndef LBM_PAIR_TY
 #define LBM_PAIR_TY 64
 #endif
+#ifndef LBM_PACK_QUAD
+#define LBM_PACK_QUAD 0   // PACK schedule in fp32 with 4 nodes per lane and per compacted group: measured no faster
+#endif
 #ifndef LBM_PAIR_QUAD
 #define LBM_PAIR_QUAD 0   // 4 nodes per lane in fp32: measured equal to 2 (0.96 vs 0.97 ms), kept as a build knob
 #endif
@@ -220,7 +223,6 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   using L = LaneOf<V>;
   using R = typename L::R;
   using Ring = PairRing<V, DP, PACKED>;
-  static_assert(!PACKED || L::NL == 2, "the PACK schedule compacts node pairs");
   constexpr int NL = L::NL;
   constexpr int OUTC = 30 * NL;            // output columns of a strip
   constexpr unsigned FULL = 0xffffffffu;
@@ -245,8 +247,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   const bool col_out = lane >= 1 && lane <= 30 && lxa < xend;
   int xa = lxa % nx;                                     // every lane is a valid periodic group
   if (xa < 0) xa += nx;
-  const int pword = (xa / 2) >> 5;                       // PACK: word and bit of the lane's pair in ptab
-  const unsigned pbit = (unsigned)(xa / 2) & 31u, plt = (1u << pbit) - 1u;
+  const int pword = (xa / NL) >> 5;                      // PACK: word and bit of the lane's group in ptab
+  const unsigned pbit = (unsigned)(xa / NL) & 31u, plt = (1u << pbit) - 1u;
   // lanes whose groups share a 32-byte sector of a population plane (rows keep the sector phase only
   // if the row pitch is a multiple of 32 bytes); a sector that holds any fluid node is stored whole
   // (zeros on its solid nodes), so that HBM never has to read-modify-write a partial sector
@@ -282,7 +284,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       if (PACKED) {
         const uint2 tb = S.Tb[sc][lane];
         const unsigned ci = tb.y + (unsigned)__popc(tb.x & plt);
-        ke = ci * 2u;
+        ke = ci * (unsigned)NL;
         d += (unsigned)lane * VB;   // entry = lane (an entry aligned to the compact index was tried: no gain)
       }
       const char* src = reinterpret_cast<const char*>(Nsrc + ke);   // plane q is src + q * psB
@@ -401,7 +403,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
         unsigned ko = kout;
         if (PACKED) {
           const uint2 tb = S.Tb[sC_i][lane];
-          ko = (tb.y + (unsigned)__popc(tb.x & plt)) * 2u;
+          ko = (tb.y + (unsigned)__popc(tb.x & plt)) * (unsigned)NL;
         }
         char* dst = reinterpret_cast<char*>(Ndst + ko);
 #pragma unroll
@@ -501,7 +503,11 @@ inline bool launch_fused_pair(const Consts<float>& C, const uint16_t* cl16, cons
   return launch_fused_lane<F2, LBM_PAIR_DP32, LBM_PAIR_MINB32, false>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st);
 }
 
-// PACK schedule: the same kernel on pair-compacted planes (Nsrc / Ndst are the compact buffers)
+// nodes per compacted group of the PACK schedule: the kernel's nodes per lane (4 in fp32 when the quad
+// variant is enabled and nx allows it, else 2)
+inline int pack_group(int elem_size, int nx) { return (elem_size == 4 && LBM_PACK_QUAD && (nx & 3) == 0) ? 4 : 2; }
+
+// PACK schedule: the same kernel on group-compacted planes (Nsrc / Ndst are the compact buffers)
 inline bool launch_fused_pack(const Consts<double>& C, const uint16_t* cl16, const double* Nsrc, double* Ndst,
                               double* Bdst, const double* phi_in, double* phi_out, cudaStream_t st,
                               const uint2* ptab, int nw, unsigned cpsB) {
@@ -510,6 +516,8 @@ inline bool launch_fused_pack(const Consts<double>& C, const uint16_t* cl16, con
 inline bool launch_fused_pack(const Consts<float>& C, const uint16_t* cl16, const float* Nsrc, float* Ndst,
                               float* Bdst, const float* phi_in, float* phi_out, cudaStream_t st,
                               const uint2* ptab, int nw, unsigned cpsB) {
+  if (pack_group(4, C.nx) == 4)
+    return launch_fused_lane<Q4, LBM_PAIR_DP32, LBM_PAIR_MINBQ, true>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st, ptab, nw, cpsB);
   return launch_fused_lane<F2, LBM_PAIR_DP32, LBM_PAIR_MINB32, true>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, st, ptab, nw, cpsB);
 }
 
