@@ -174,8 +174,13 @@ __device__ __forceinline__ void cp_async_vec(unsigned saddr, const void* gptr) {
 
 // shared-memory ring of one warp: row stages hold the own-position populations and phi of the strip;
 // class stages the packed class words (NL 16-bit words per lane)
+// PACK schedule only: {group mask word, compact index of its first group} per class row.  Kept out of
+// the ring of the other schedules: 3 CTAs x 64 KB is the most that fits the 196 KB shared-memory carve-out,
+// one KB more selects the 228 KB carve-out, halves L1 and costs 30 % (LDGSTS allocates its lines in L1).
+template <int CS, bool PACKED> struct RingTab { uint2 Tb[CS][32]; };
+template <int CS> struct RingTab<CS, false> {};
 template <typename V, int DP, bool PACKED>
-struct PairRing {
+struct PairRing : RingTab<2 * DP + 2, PACKED> {
   static constexpr int NL = LaneOf<V>::NL;
   static constexpr int NS = DP + 2;        // population rows i-1 (until refilled) .. i+1+DP
   static constexpr int PS = DP + 3;        // phi rows i-1 .. i+1+DP
@@ -183,7 +188,6 @@ struct PairRing {
   V N[NS][9][32];
   V P[PS][32];
   unsigned short Cw[CS][32][NL];
-  uint2 Tb[PACKED ? CS : 1][32];           // PACK schedule: {pair mask word, compact index of its first pair}
 };
 
 // collide the NL nodes of a lane (fl[c]: node c is fluid).  All nodes always go through the
@@ -234,7 +238,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   const unsigned sN0 = (unsigned)__cvta_generic_to_shared(&S.N[0][0][PACKED ? 0 : lane]);
   const unsigned sP0 = (unsigned)__cvta_generic_to_shared(&S.P[0][lane]);
   const unsigned sC0 = (unsigned)__cvta_generic_to_shared(&S.Cw[0][lane][0]);
-  const unsigned sT0 = (unsigned)__cvta_generic_to_shared(&S.Tb[0][lane]);
+  unsigned sT0 = 0;
+  if constexpr (PACKED) sT0 = (unsigned)__cvta_generic_to_shared(&S.Tb[0][lane]);
   constexpr unsigned N_STAGE = 9 * 32 * VB, N_PLANE = 32 * VB, P_STAGE = 32 * VB, C_STAGE = 32 * NL * 2;
 
   const int nx = C.nx, ny = C.ny;   // nx is a multiple of NL (checked by the launcher)
@@ -266,7 +271,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   // ---- asynchronous fetches (slots and row offsets are passed in: no modulo in the march) ----
   auto issue_cls = [&](int r, int sc) {   // the NL class words of the lane in grid row r (one aligned word)
     cp_async_vec<NL * 2>(sC0 + (unsigned)sc * C_STAGE, cl16 + ((unsigned)r * (unsigned)nx + (unsigned)xa));
-    if (PACKED) cp_async_vec<8>(sT0 + (unsigned)sc * 256u, ptab + ((size_t)r * nw + pword));
+    if constexpr (PACKED) cp_async_vec<8>(sT0 + (unsigned)sc * 256u, ptab + ((size_t)r * nw + pword));
   };
   // own-position populations and phi of one march row; lower/upper: the row feeds c_y <= 0 / c_y >= 0
   auto issue_row = [&](unsigned u, int sn, int sp, int sc, bool lower, bool upper) {
@@ -281,7 +286,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     if (cmin < 2u) {
       unsigned ke = k;                                             // element offset of the group in a plane
       unsigned d = sN0 + (unsigned)sn * N_STAGE;
-      if (PACKED) {
+      if constexpr (PACKED) {
         const uint2 tb = S.Tb[sc][lane];
         const unsigned ci = tb.y + (unsigned)__popc(tb.x & plt);
         ke = ci * (unsigned)NL;
@@ -401,7 +406,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       collide_lane<V>(C, nn, ph, fl, all_fl, ns, bs);
       if (st) {
         unsigned ko = kout;
-        if (PACKED) {
+        if constexpr (PACKED) {
           const uint2 tb = S.Tb[sC_i][lane];
           ko = (tb.y + (unsigned)__popc(tb.x & plt)) * (unsigned)NL;
         }
