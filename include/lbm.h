@@ -49,7 +49,7 @@ enum { LBM_FLUID_BULK = 0, LBM_FLUID_BOUNDARY = 1, LBM_GHOST = 2, LBM_SOLID_BULK
 
 /* launch schedules of lbm_step (same arithmetic per node, different kernel decomposition) */
 enum {
-  LBM_SCHEDULE_AUTO = 0,      /* the fastest schedule available (currently PAIR)                  */
+  LBM_SCHEDULE_AUTO = 0,      /* the fastest schedule available (currently PACK)                  */
   LBM_SCHEDULE_BASELINE = 1,  /* 3 launches/step: collide+stream, phi = sum B, ghost; N and B in HBM */
   LBM_SCHEDULE_FUSED = 2,     /* 2 launches/step: tiled collide+stream that also produces phi(t+1)
                                  from B* held in shared memory (B never touches HBM), ghost        */

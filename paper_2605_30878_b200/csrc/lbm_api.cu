@@ -180,7 +180,9 @@ bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELIN
 // one layout function serves both sizing (base == nullptr) and carving; everything that does not
 // depend on the ghost count comes first, so a carve with ng = 0 and one with the real ng agree
 // on those arrays
-bool use_pack(const lbm_params* P) { return P->schedule == LBM_SCHEDULE_PACK && (P->nx % 2) == 0; }
+bool use_pack(const lbm_params* P) {
+  return (P->schedule == LBM_SCHEDULE_PACK || P->schedule == LBM_SCHEDULE_AUTO) && (P->nx % 2) == 0;
+}
 
 // number of aligned node pairs that hold a fluid node (PACK schedule); mask: host, non-zero = solid
 long long count_fluid_pairs(const lbm_params* P, const uint8_t* mask) {
@@ -437,7 +439,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   c->n = n;
   c->is32 = prm->precision == 32;
   c->fused = use_fused(prm) ? 1 : 0;
-  c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? LBM_SCHEDULE_PAIR : prm->schedule;
+  c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? (use_pack(prm) ? LBM_SCHEDULE_PACK : LBM_SCHEDULE_PAIR) : prm->schedule;
   c->st = (cudaStream_t)cuda_stream;
   c->Cd = make_consts<double>(*prm);
   c->Cf = make_consts<float>(*prm);

@@ -49,14 +49,18 @@ namespace lbm {
 #ifndef LBM_PAIR_SECTOR
 #define LBM_PAIR_SECTOR 32   // bytes of the write granule that is completed with zeros
 #endif
+#ifndef LBM_PAIR_CG16
+#define LBM_PAIR_CG16 1   // 16-byte cp.async bypasses L1 (.cg): LDGSTS.ca parks its lines in L1, whose size
+                          // (what the shared-memory carve-out leaves) then caps the bytes in flight
+#endif
 #ifndef LBM_PAIR_TY
 #define LBM_PAIR_TY 64
 #endif
 #ifndef LBM_PACK_QUAD
-#define LBM_PACK_QUAD 0   // PACK schedule in fp32 with 4 nodes per lane and per compacted group: measured no faster
+#define LBM_PACK_QUAD 1   // PACK schedule in fp32: 4 nodes per lane and per compacted group (16-byte copies)
 #endif
 #ifndef LBM_PAIR_QUAD
-#define LBM_PAIR_QUAD 0   // 4 nodes per lane in fp32: measured equal to 2 (0.96 vs 0.97 ms), kept as a build knob
+#define LBM_PAIR_QUAD 1   // PAIR schedule in fp32: 4 nodes per lane when nx % 4 == 0 (16-byte copies can bypass L1)
 #endif
 
 // ---- lane value types: NL nodes of one lane ----
@@ -168,7 +172,14 @@ __device__ __forceinline__ void store_vec(void* p, V v) {
 
 template <int BYTES>
 __device__ __forceinline__ void cp_async_vec(unsigned saddr, const void* gptr) {
-  // .ca for every size: with .cg (L1 bypass) the two 16-byte lanes of a sector each fetch it from L2
+  // 4- and 8-byte copies exist only as .ca; 16-byte copies bypass L1 (.cg): each sector then crosses the
+  // L2 -> SM link once per 16-byte lane, but L1 capacity no longer limits how many rows are in flight
+#if LBM_PAIR_CG16
+  if constexpr (BYTES == 16) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gptr) : "memory");
+    return;
+  }
+#endif
   asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(saddr), "l"(gptr), "n"(BYTES) : "memory");
 }
 
@@ -488,6 +499,9 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   static bool attr_set[2] = {false, false};
   if (!attr_set[Bdst ? 1 : 0]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+#ifdef LBM_PAIR_CARVEOUT
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, LBM_PAIR_CARVEOUT);   // tuning experiment
+#endif
     attr_set[Bdst ? 1 : 0] = true;
   }
   kern<<<grid, 32 * WARPS, smem, st>>>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, TY, ptab, nw, cpsB);
