@@ -32,16 +32,16 @@ namespace lbm {
 #define LBM_PAIR_DP64 1
 #endif
 #ifndef LBM_PAIR_MINB32
-#define LBM_PAIR_MINB32 4
+#define LBM_PAIR_MINB32 5
 #endif
 #ifndef LBM_PAIR_MINB64
-#define LBM_PAIR_MINB64 3
+#define LBM_PAIR_MINB64 4
 #endif
 #ifndef LBM_PAIR_MINBQ
-#define LBM_PAIR_MINBQ 3
+#define LBM_PAIR_MINBQ 4
 #endif
 #ifndef LBM_PAIR_WARPS
-#define LBM_PAIR_WARPS 4
+#define LBM_PAIR_WARPS 3
 #endif
 #ifndef LBM_PAIR_FULLSECTOR
 #define LBM_PAIR_FULLSECTOR 1
