@@ -569,10 +569,14 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
       k_pair_tab<<<nb, 256, 0, c->st>>>(pmask, pbase, nwords, c->ptab);
       e = cudaGetLastError();
     }
+    int last[2] = {0, 0};   // the device's group count must be the host's (the compact planes were sized with it)
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&last[0], pbase + (nwords - 1), sizeof(int), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&last[1], pcount + (nwords - 1), sizeof(int), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
     cudaFree(tmp);
     cudaFree(pmask);
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "pair table"); }
+    if ((long long)last[0] + last[1] != nfp) { delete c; return fail(nullptr, LBM_EINVAL, "internal: fluid group counts of host and device differ"); }
     c->packed = 1;
   }
   CKC(cudaStreamSynchronize(c->st));
