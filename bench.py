@@ -253,8 +253,8 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=2000, help="timed steps (BASELINE config 5: 2,000)")
+    ap.add_argument("--warmup", type=int, default=50, help="untimed warm-up steps (SURVEY 8(d): >= 50)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=8192)
     ap.add_argument("--precision", default="both", choices=["64", "32", "both"])
