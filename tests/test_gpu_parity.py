@@ -498,3 +498,20 @@ def test_layout_copy_helper_leaves_the_state_alone():
     assert ms_copy > 0
     for k in a:
         assert np.array_equal(b[k], c[k]), k            # same as a run without the helper, bit for bit
+
+
+@pytest.mark.parametrize("schedule", [pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack")])
+@pytest.mark.parametrize("shape,frac", [((7, 4), 0.2), ((9, 12), 0.3), ((33, 36), 0.3), ((50, 100), 0.25),
+                                        ((61, 244), 0.3), ((40, 126), 0.3)])
+def test_random_masks_ragged_fp32(schedule, shape, frac):
+    """fp32 lane groups: four nodes per lane when nx % 4 == 0, two otherwise, strips wider than the grid."""
+    w = _random_case(shape[0], shape[1], seed=shape[0] * 1000 + shape[1], frac=frac, rho_l=20.0, nu_l=0.05)
+    g, o = make_pair(w, precision=32, schedule=schedule)
+    g.init(w.phi0); o.init(w.phi0)
+    g.step(20); o.step(20)
+    err, scale = field_errors(g, o)
+    uscale = max(scale["ux"], scale["uy"], w.prm["sigma"] / (w.prm["rho_l"] * w.prm["nu_l"]))
+    assert err["phi"] <= 2e-4 and max(err["ux"], err["uy"]) <= 2e-4 * uscale, err
+    Ng, _ = g.get_populations(want_B=False)
+    No, _ = o.get_populations()
+    assert np.abs(Ng - No)[:, w.mask == 0].max() <= 2e-4
