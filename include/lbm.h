@@ -60,11 +60,16 @@ enum {
                                  population is fetched once, unshifted, as an 8/16-byte vector;
                                  propagation in x is a warp shuffle; fp32 arithmetic is packed
                                  (FFMA2).  Needs even nx, else FUSED is used                        */
-  LBM_SCHEDULE_PACK = 5       /* the PAIR kernel on pair-compacted population planes: a plane stores
+  LBM_SCHEDULE_PACK = 5,      /* the PAIR kernel on pair-compacted population planes: a plane stores
                                  only the node pairs that hold a fluid node, row after row, without
                                  holes (addressed through a 1-bit-per-pair mask + prefix table).  The
                                  dense planes are kept as a mirror that lbm_get / lbm_diag / ... refresh
                                  on demand.  Needs even nx, else FUSED is used                      */
+  LBM_SCHEDULE_SPARSE = 6     /* the PACK layout with lanes mapped to fluid groups: one persistent CTA
+                                 per SM, rows brought on chip by 1-D bulk copies (TMA) into a shared-memory
+                                 ring, consumer warps work on 32 consecutive entries of the active-group
+                                 sequence.  Needs 16-byte groups (fp64: even nx; fp32: nx % 4 == 0) and
+                                 at least 4 groups per row, else PACK is used                        */
 };
 
 typedef struct lbm_ctx lbm_ctx;                 /* opaque; one simulation                         */

@@ -19,7 +19,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 _SO = os.path.join(_HERE, "liblbm_b200.so")
 
-SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_WARP, SCHEDULE_PAIR, SCHEDULE_PACK = 0, 1, 2, 3, 4, 5
+SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_WARP, SCHEDULE_PAIR, SCHEDULE_PACK, SCHEDULE_SPARSE = 0, 1, 2, 3, 4, 5, 6
 FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
 EXPORTS = ("lbm_plan", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",

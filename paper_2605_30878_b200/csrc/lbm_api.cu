@@ -7,6 +7,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -14,6 +15,7 @@
 #include "lbm_fused.cuh"
 #include "lbm_kernels.cuh"
 #include "lbm_pair.cuh"
+#include "lbm_sparse.cuh"
 #include "lbm_warp.cuh"
 
 using namespace lbm;
@@ -74,6 +76,15 @@ struct lbm_ctx {
   size_t cps;        // compact plane stride in pairs
   uint2* ptab;
   void* Nc[2];
+  // SPARSE schedule: per (strip, row) descriptors, per-group metadata, the marches of every CTA
+  int sparse;
+  int sp_nstrips, sp_ncta, sp_nmarch;
+  SpDesc* sp_desc;
+  uint16_t* sp_cnt;
+  uint2* sp_meta;
+  SpMarch* sp_march;
+  int* sp_first;
+  size_t sp_march_cap;
   int* blk_cnt;
   int* blk_off;
   int* scal;          // [0] ghost total, [1] geometry error flag
@@ -122,7 +133,7 @@ int validate(const lbm_params* P, const char** why) {
   if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
   if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
   if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
-  if (P->schedule < 0 || P->schedule > 5) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 6) { *why = "unknown schedule"; return LBM_EINVAL; }
   if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
   return LBM_OK;
 }
@@ -181,7 +192,24 @@ bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELIN
 // depend on the ghost count comes first, so a carve with ng = 0 and one with the real ng agree
 // on those arrays
 bool use_pack(const lbm_params* P) {
-  return (P->schedule == LBM_SCHEDULE_PACK || P->schedule == LBM_SCHEDULE_AUTO) && (P->nx % 2) == 0;
+  return (P->schedule == LBM_SCHEDULE_PACK || P->schedule == LBM_SCHEDULE_AUTO || P->schedule == LBM_SCHEDULE_SPARSE) &&
+         (P->nx % 2) == 0;
+}
+// SPARSE runs on the PACK layout when a group is 16 bytes (fp64 pairs, fp32 quads) and a row has enough groups
+// for the two-group phi halo of a strip to wrap at most once
+constexpr int kSpMaxCta = 1024;
+bool use_sparse(const lbm_params* P) {
+  if (P->schedule != LBM_SCHEDULE_SPARSE || !use_pack(P)) return false;
+  const int G = pack_group(P->precision == 32 ? 4 : 8, P->nx);
+  const int ng = P->nx / G;
+  return G * (P->precision == 32 ? 4 : 8) == 16 && ng >= 4 && ng <= 65535;
+}
+int sp_strips(const lbm_params* P) {
+  const int ng = P->nx / pack_group(P->precision == 32 ? 4 : 8, P->nx);
+  return (ng + SP_S - 1) / SP_S;
+}
+size_t sp_march_capacity(const lbm_params* P) {
+  return (size_t)sp_strips(P) * ((size_t)P->ny / SP_TYMAX + 2) + kSpMaxCta + 8;
 }
 
 // number of aligned node pairs that hold a fluid node (PACK schedule); mask: host, non-zero = solid
@@ -244,7 +272,18 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
     Nc0 = A.take<char>(9 * cps * G * rs);
     Nc1 = A.take<char>(9 * cps * G * rs);
   }
+  SpDesc* sp_desc = nullptr; uint16_t* sp_cnt = nullptr; uint2* sp_meta = nullptr; SpMarch* sp_march = nullptr; int* sp_first = nullptr;
+  if (use_sparse(P)) {
+    const size_t nsr = (size_t)sp_strips(P) * P->ny;
+    sp_desc = A.take<SpDesc>(nsr);
+    sp_cnt = A.take<uint16_t>(nsr + 8);
+    sp_meta = A.take<uint2>((size_t)(nfp > 0 ? nfp : 1) + 64);
+    sp_march = A.take<SpMarch>(sp_march_capacity(P));
+    sp_first = A.take<int>(kSpMaxCta + 8);
+  }
   if (c && base) {
+    c->sp_desc = sp_desc; c->sp_cnt = sp_cnt; c->sp_meta = sp_meta; c->sp_march = sp_march; c->sp_first = sp_first;
+    c->sp_march_cap = sp_march_capacity(P);
     c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
     c->cls = cls; c->links = links; c->cl16 = cl16; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
     c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid;
@@ -297,6 +336,9 @@ void launch_ghost(lbm_ctx* c) {
   c->launches[2]++;
 }
 
+bool launch_fused_sparse(lbm_ctx* c, const Consts<double>& C, const double* Ns, double* Nd, double* Bd, const double* pi, double* po);
+bool launch_fused_sparse(lbm_ctx* c, const Consts<float>& C, const float* Ns, float* Nd, float* Bd, const float* pi, float* po);
+
 struct StepTimer {   // optional event brackets around each launch (lbm_step_timed)
   cudaEvent_t ev[4];
   double ms[3];
@@ -326,7 +368,13 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     const R* pi = (const R*)c->phi[c->pcur];
     R* po = (R*)c->phi[c->pcur ^ 1];
     bool done = false;
-    if (c->packed) {   // PACK: compact planes step compact -> compact; the dense mirror N[cur] goes stale
+    if (c->packed && c->sparse) {   // SPARSE: the same compact planes, lanes mapped to fluid groups
+      done = launch_fused_sparse(c, C, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po);
+      if (!done) return LBM_ECUDA;
+      c->ccur ^= 1;
+      c->dense_valid = 0;
+      c->cur ^= 1;     // undone below: the dense buffer index does not move
+    } else if (c->packed) {   // PACK: compact planes step compact -> compact; the dense mirror N[cur] goes stale
       done = launch_fused_pack(C, c->cl16, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po, c->st, c->ptab,
                                c->nw, (unsigned)(c->cps * pack_group((int)sizeof(R), c->P.nx) * sizeof(R)));
       c->ccur ^= 1;
@@ -355,6 +403,59 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     tm->ms[0] += a; tm->ms[1] += b; tm->ms[2] += g;
   }
   return LBM_OK;
+}
+
+
+// SPARSE schedule: one persistent CTA per SM (lbm_sparse.cuh)
+template <typename V, typename R>
+bool launch_sparse_v(lbm_ctx* c, const Consts<R>& C, const R* Ns, R* Nd, R* Bd, const R* pi, R* po) {
+  const size_t smem = sizeof(SpSmem<V>);
+  auto kern = Bd ? k_fused_sparse<V, true> : k_fused_sparse<V, false>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+  const unsigned cpsB = (unsigned)(c->cps * 16);
+  kern<<<c->sp_ncta, SP_THREADS, smem, c->st>>>(C, Ns, Nd, Bd, pi, po, c->sp_desc, c->sp_cnt, c->sp_meta, c->sp_march,
+                                               c->sp_first, cpsB);
+  return true;
+}
+bool launch_fused_sparse(lbm_ctx* c, const Consts<double>& C, const double* Ns, double* Nd, double* Bd, const double* pi,
+                         double* po) {
+  return launch_sparse_v<D2, double>(c, C, Ns, Nd, Bd, pi, po);
+}
+bool launch_fused_sparse(lbm_ctx* c, const Consts<float>& C, const float* Ns, float* Nd, float* Bd, const float* pi,
+                         float* po) {
+  return launch_sparse_v<Q4, float>(c, C, Ns, Nd, Bd, pi, po);
+}
+
+// SPARSE schedule, one-time: cut the (strip, row) sequence into marches of about equal weight, one run of
+// marches per CTA.  cnt[strip * ny + row] = entries of that strip row.
+void sp_partition(const uint16_t* cnt, int nstrips, int ny, int ncta_max, std::vector<SpMarch>& marches,
+                  std::vector<int>& first) {
+  double total = 0.0;
+  auto weight = [&](int s, int r) { return (double)std::max<int>(cnt[(size_t)s * ny + r], SP_MINPOS) + 4.0; };
+  for (int s = 0; s < nstrips; s++)
+    for (int r = 0; r < ny; r++) total += weight(s, r);
+  // a CTA should have at least ~64 rows of a full strip to amortise its 4 halo rows
+  int ncta = (int)std::min<double>(ncta_max, std::max(1.0, total / (64.0 * (SP_S + 4))));
+  const double target = total / ncta;
+  marches.clear();
+  first.assign(1, 0);
+  double cum = 0.0;
+  int cur = 0;
+  for (int s = 0; s < nstrips; s++) {
+    int r = 0;
+    while (r < ny) {
+      const int owner = std::min(ncta - 1, (int)(cum / target));
+      while (cur < owner) { first.push_back((int)marches.size()); cur++; }
+      SpMarch m{s, r, 0, 0};
+      while (r < ny && m.rows < SP_TYMAX && std::min(ncta - 1, (int)(cum / target)) == owner) {
+        cum += weight(s, r);
+        r++;
+        m.rows++;
+      }
+      marches.push_back(m);
+    }
+  }
+  while (cur < ncta) { first.push_back((int)marches.size()); cur++; }
 }
 
 // PACK schedule: refresh the dense mirror N[cur] from the compact planes before a dense reader runs
@@ -440,6 +541,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   c->is32 = prm->precision == 32;
   c->fused = use_fused(prm) ? 1 : 0;
   c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? (use_pack(prm) ? LBM_SCHEDULE_PACK : LBM_SCHEDULE_PAIR) : prm->schedule;
+  if (c->sched == LBM_SCHEDULE_SPARSE && !use_sparse(prm)) c->sched = use_pack(prm) ? LBM_SCHEDULE_PACK : LBM_SCHEDULE_PAIR;
   c->st = (cudaStream_t)cuda_stream;
   c->Cd = make_consts<double>(*prm);
   c->Cf = make_consts<float>(*prm);
@@ -578,6 +680,34 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "pair table"); }
     if ((long long)last[0] + last[1] != nfp) { delete c; return fail(nullptr, LBM_EINVAL, "internal: fluid group counts of host and device differ"); }
     c->packed = 1;
+  }
+  if (use_sparse(prm)) {   // SPARSE schedule: per-group metadata, per (strip, row) descriptors, marches
+    const int G = pack_group(c->is32 ? 4 : 8, prm->nx);
+    const int ng = prm->nx / G;
+    const int nstrips = sp_strips(prm);
+    const size_t nsr = (size_t)nstrips * prm->ny;
+    k_sp_meta<<<(unsigned)(((long long)prm->ny * ng + 255) / 256), 256, 0, c->st>>>(c->cls, c->links, c->ptab, prm->nx, prm->ny,
+                                                                                 c->nw, G, c->sp_meta);
+    k_sp_desc<<<(unsigned)((nsr + 127) / 128), 128, 0, c->st>>>(c->ptab, c->sp_meta, prm->nx, prm->ny, c->nw, G, nstrips,
+                                                               c->sp_desc, c->sp_cnt);
+    CKC(cudaGetLastError());
+    std::vector<uint16_t> h_cnt(nsr);
+    CKC(cudaMemcpyAsync(h_cnt.data(), c->sp_cnt, nsr * sizeof(uint16_t), cudaMemcpyDeviceToHost, c->st));
+    CKC(cudaStreamSynchronize(c->st));
+    int dev = 0, nsm = 0;
+    CKC(cudaGetDevice(&dev));
+    CKC(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    std::vector<SpMarch> marches;
+    std::vector<int> first;
+    sp_partition(h_cnt.data(), nstrips, prm->ny, std::min(nsm, kSpMaxCta), marches, first);
+    if (marches.size() > c->sp_march_cap) { delete c; return fail(nullptr, LBM_EINVAL, "internal: march table overflow"); }
+    CKC(cudaMemcpyAsync(c->sp_march, marches.data(), marches.size() * sizeof(SpMarch), cudaMemcpyHostToDevice, c->st));
+    CKC(cudaMemcpyAsync(c->sp_first, first.data(), first.size() * sizeof(int), cudaMemcpyHostToDevice, c->st));
+    CKC(cudaStreamSynchronize(c->st));
+    c->sp_nstrips = nstrips;
+    c->sp_ncta = (int)first.size() - 1;
+    c->sp_nmarch = (int)marches.size();
+    c->sparse = 1;
   }
   CKC(cudaStreamSynchronize(c->st));
 #undef CKC

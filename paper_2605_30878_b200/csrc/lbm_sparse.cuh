@@ -1,0 +1,605 @@
+// lbm_sparse.cuh — SPARSE schedule: the fused pull-stream + collide + segregation + phi(t+1) kernel with
+// lanes mapped to FLUID GROUPS instead of columns.
+//
+// State: the group-compacted planes of the PACK schedule (lbm_kernels.cuh: k_pair_mask, ptab) — a plane
+// stores only the aligned groups of NL x-adjacent nodes that hold a fluid node, row after row.  What
+// changes is who works on what:
+//
+//   * one persistent CTA per SM owns "marches": a strip of SP_S groups, a run of rows.  A row of a strip is
+//     a CONTIGUOUS run of the compact planes, so one producer warp brings every row on chip with eleven
+//     1-D bulk copies (cp.async.bulk -> UBLKCP, complete_tx on an mbarrier): nine population planes, the
+//     per-group metadata, the dense phi row.  Rows live in a shared-memory ring sized in entries, not rows.
+//   * the SP_W consumer warps take "passes": 32 consecutive ENTRIES of the row-major sequence of the
+//     strip's active groups (a pass may span several rows; 30 outputs + one helper lane per side).  Every
+//     lane therefore holds a group with a fluid node: no issue slot is spent on solid lanes.
+//   * propagation (A16-A17) is a gather from the ring: same-row neighbours are the adjacent entries, the
+//     groups above / below are found by popcount on the row's group mask.  Half-way bounce-back (R12)
+//     selects the node's own opposite population, as in the PAIR kernel.
+//   * phi(x, t+1) = sum_q B_q*(x - c_q, t) (A13): every output lane writes the three partial sums its row
+//     sends to the rows above / at / below (x-moves by warp shuffle between x-adjacent lanes) into dense
+//     per-row buffers, each address written by exactly one lane; the producer warp adds the three rows
+//     once all consumers are past them and stores phi(t+1).  No atomics: results are run-to-run identical.
+//   * synchronisation: one mbarrier per row slot (producer -> consumers, TMA transaction bytes), one
+//     monotone "last row I am done with" counter per consumer warp (consumers -> producer) and one
+//     monotone counter for the partial-sum buffers.  No __syncthreads inside a march.
+#pragma once
+#include "lbm_pair.cuh"
+
+namespace lbm {
+
+#ifndef LBM_SP_WARPS
+#define LBM_SP_WARPS 12
+#endif
+#ifndef LBM_SP_CAP
+#define LBM_SP_CAP 832
+#endif
+constexpr int SP_S = 126;                 // body groups of a strip; S + 2 halo groups = 128 mask bits
+constexpr int SP_W = LBM_SP_WARPS;        // consumer warps (+ 1 producer warp)
+constexpr int SP_NR = 16;                 // row slots (phi rows, row info, full barriers)
+constexpr int SP_NRU = 8;                 // row slots of the partial-sum buffers
+constexpr int SP_CAP = LBM_SP_CAP;        // entries of the population ring
+constexpr int SP_TYMAX = 512;             // rows of a march
+constexpr int SP_MINPOS = 8;              // a row takes at least this many positions of the pass sequence, so
+                                          // that a pass of 32 positions spans at most 5 rows
+constexpr int SP_THREADS = 32 * (SP_W + 1);
+
+// per (strip, row) descriptor, built once by k_sp_desc
+struct __align__(16) SpDesc {
+  uint32_t ci0;       // compact index of the strip's first body group in this row (insertion point if absent)
+  uint32_t ciL, ciR;  // compact indices of the halo groups left / right of the body (valid if hl / hr)
+  uint16_t a;         // active body groups
+  uint8_t hl, hr;     // halo group active
+  uint32_t bits[4];   // bit c + 1 set <=> group c of the strip holds a fluid node, c = -1 .. S
+  uint2 metaL, metaR; // metadata of the halo groups
+  uint8_t pre[4];     // popcount of the words below
+  uint32_t pad[3];
+};
+static_assert(sizeof(SpDesc) == 64, "descriptor layout");
+
+// per compact group: x = column of the group | fluid bits << 16 | left neighbour group active << 20 |
+// right neighbour group active << 21; y = bounce-back link byte of each node
+struct SpMarch { int strip, j0, rows, pad; };
+
+struct SpRow {        // shared-memory copy of what the consumers need of a row
+  uint32_t off;       // ring index of entry 0
+  uint32_t ci0;       // compact index of the first body entry
+  uint32_t n;         // entries: hl + a + hr
+  uint32_t hlr;       // bit 0: left halo entry present, bit 1: right halo entry present
+  uint32_t bits[4];
+  uint32_t pre;       // four prefix bytes
+  uint32_t jrow;      // grid row
+  uint2 metaL, metaR;
+};
+
+template <typename V>
+struct SpSmem {
+  V N[9][SP_CAP];
+  uint2 meta[SP_CAP];
+  V phi[SP_NR][SP_S + 4];
+  V U[SP_NRU][SP_S + 2];
+  V M[SP_NRU][SP_S + 2];
+  V D[SP_NRU][SP_S + 2];
+  SpRow row[SP_NR];
+  uint32_t T[SP_TYMAX + 4];
+  unsigned long long full[SP_NR];
+  int rstart[SP_NR];
+  int done[32];
+  int um_ready;
+  int pad[3];
+};
+
+// ---- mbarrier / bulk-copy / ordered shared-memory access ----
+__device__ __forceinline__ void mbar_init(unsigned a, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_inval(unsigned a) {
+  asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_tx(unsigned a, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(unsigned a, unsigned parity) {
+  unsigned ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(a), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+// a wait that cannot hang the device: a schedule bug traps instead (reported as a CUDA error by lbm_step)
+__device__ __forceinline__ void mbar_wait(unsigned a, unsigned parity) {
+  if (mbar_test(a, parity)) return;
+  const long long t0 = clock64();
+  while (!mbar_test(a, parity))
+    if (clock64() - t0 > 8000000000LL) __trap();
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(mbar)
+               : "memory");
+}
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"((unsigned)__cvta_generic_to_shared(p)) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v) {
+  asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void wait_counter(const int* p, int target) {
+  if (ld_acquire(p) >= target) return;
+  const long long t0 = clock64();
+  while (ld_acquire(p) < target) {
+    __nanosleep(64);
+    if (clock64() - t0 > 8000000000LL) __trap();
+  }
+}
+
+// a lane's vector with one scalar shifted in from the left / right neighbour node
+template <typename V>
+__device__ __forceinline__ V shift_in_left(V own, typename LaneOf<V>::R s) {
+  using L = LaneOf<V>;
+  typename L::R x[L::NL], y[L::NL];
+  L::unpack(own, x);
+  y[0] = s;
+#pragma unroll
+  for (int c = 1; c < L::NL; c++) y[c] = x[c - 1];
+  return L::pack(y);
+}
+template <typename V>
+__device__ __forceinline__ V shift_in_right(V own, typename LaneOf<V>::R s) {
+  using L = LaneOf<V>;
+  typename L::R x[L::NL], y[L::NL];
+  L::unpack(own, x);
+#pragma unroll
+  for (int c = 0; c < L::NL - 1; c++) y[c] = x[c + 1];
+  y[L::NL - 1] = s;
+  return L::pack(y);
+}
+template <typename V>
+__device__ __forceinline__ typename LaneOf<V>::R first_of(V v) {
+  typename LaneOf<V>::R x[LaneOf<V>::NL];
+  LaneOf<V>::unpack(v, x);
+  return x[0];
+}
+template <typename V>
+__device__ __forceinline__ typename LaneOf<V>::R last_of(V v) {
+  typename LaneOf<V>::R x[LaneOf<V>::NL];
+  LaneOf<V>::unpack(v, x);
+  return x[LaneOf<V>::NL - 1];
+}
+
+// entry index, within its row, of group c (c = -1 .. S): the number of active groups with a smaller column
+__device__ __forceinline__ int sp_rank(const SpRow& r, int c, unsigned* bit) {
+  const unsigned b = (unsigned)(c + 1);
+  const unsigned w = r.bits[b >> 5];
+  *bit = (w >> (b & 31u)) & 1u;
+  return (int)((r.pre >> (8u * (b >> 5))) & 0xffu) + __popc(w & ((1u << (b & 31u)) - 1u));
+}
+
+template <typename V, bool WRITE_B>
+__global__ void __launch_bounds__(SP_THREADS, 1)
+    k_fused_sparse(const Consts<typename LaneOf<V>::R> C, const typename LaneOf<V>::R* __restrict__ Nsrc,
+                   typename LaneOf<V>::R* __restrict__ Ndst, typename LaneOf<V>::R* __restrict__ Bdst,
+                   const typename LaneOf<V>::R* __restrict__ phi_in, typename LaneOf<V>::R* __restrict__ phi_out,
+                   const SpDesc* __restrict__ desc, const uint16_t* __restrict__ cnt, const uint2* __restrict__ gmeta,
+                   const SpMarch* __restrict__ marches, const int* __restrict__ cta_first, unsigned cpsB) {
+  using L = LaneOf<V>;
+  using R = typename L::R;
+  constexpr int NL = L::NL;
+  constexpr unsigned FULL = 0xffffffffu;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SpSmem<V>& S = *reinterpret_cast<SpSmem<V>*>(smem_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nx = C.nx, ny = C.ny;
+  const int ng = nx / NL;                                      // groups per row
+  const unsigned psBd = (unsigned)C.ps * (unsigned)sizeof(R);  // dense plane stride in bytes (B planes)
+  const V zero = splat<V>(R(0));
+
+  // stale ring entries are read (and discarded, or multiplied by a zero mask): they must be finite
+  for (int k = tid; k < 9 * SP_CAP; k += SP_THREADS) (&S.N[0][0])[k] = zero;
+  for (int k = tid; k < SP_NR * (SP_S + 4); k += SP_THREADS) (&S.phi[0][0])[k] = zero;
+  for (int k = tid; k < SP_CAP; k += SP_THREADS) S.meta[k] = make_uint2(0u, 0u);
+
+  for (int mi = cta_first[blockIdx.x]; mi < cta_first[blockIdx.x + 1]; mi++) {
+    const SpMarch mar = marches[mi];
+    const int c0 = mar.strip * SP_S;                           // first body group of the strip
+    const int seff = min(SP_S, ng - c0);                       // body groups of this strip
+    const int TY = mar.rows;
+    const int nR = TY + 4;                                     // ring rows R = 0 .. TY+3 <-> grid rows j0-2 ..
+    const SpDesc* sdesc = desc + (size_t)mar.strip * ny;
+    const uint16_t* scnt = cnt + (size_t)mar.strip * ny;
+    auto grid_row = [&](int Rr) -> int {
+      int j = mar.j0 - 2 + Rr;
+      j %= ny;
+      return j < 0 ? j + ny : j;
+    };
+    __syncthreads();   // previous march finished; zero fill visible
+    // ---- pass sequence: T[k] = positions of processed rows R = 1 .. k (k = 0 .. TY+2) ----
+    if (warp == 0) {
+      unsigned run = 0;
+      for (int base = 0; base < TY + 2; base += 32) {
+        const int k = base + lane;
+        unsigned v = 0;
+        if (k < TY + 2) v = max((unsigned)scnt[grid_row(k + 1)], (unsigned)SP_MINPOS);
+        unsigned s = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const unsigned t = __shfl_up_sync(FULL, s, d);
+          if (lane >= d) s += t;
+        }
+        if (k < TY + 2) S.T[k + 1] = run + s;
+        run += __shfl_sync(FULL, s, 31);
+      }
+      if (lane == 0) S.T[0] = 0;
+    }
+    if (tid == 32) {
+      for (int k = 0; k < SP_NR; k++) mbar_init((unsigned)__cvta_generic_to_shared(&S.full[k]), 1);
+      S.um_ready = 0;
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid < 32) S.done[tid] = 0;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    const int P = (int)S.T[TY + 2];
+    const int NP = (P + 29) / 30;
+
+    if (warp == SP_W) {
+      // =============================== producer / finaliser warp ===============================
+      int Rload = 0, Rret = 0, Rum = 1, head = 0;
+      SpDesc dn = sdesc[grid_row(0)];
+      while (Rret < nR) {
+        // (a) retire the oldest row if every consumer is past it
+        int mind = 0x7fffffff;
+        {
+          const int v = lane < SP_W ? ld_acquire(&S.done[lane]) : 0x7fffffff;
+          mind = v;
+#pragma unroll
+          for (int d = 16; d >= 1; d >>= 1) mind = min(mind, __shfl_xor_sync(FULL, mind, d));
+        }
+        const bool can_retire = Rret < Rload && mind >= min(Rret + 1, TY + 2);
+        // (b) partial-sum buffers of processed row Rum: free once finalise(Rum - NRU + 1) is done
+        const bool can_um = Rum <= TY + 2 && (Rum - SP_NRU < 1 || Rret >= Rum - SP_NRU + 2);
+        if (can_retire) {
+          const int Rr = Rret;
+          if (Rr >= 2 && Rr <= TY + 1) {   // phi(t+1) of row Rr = U[Rr-1] + M[Rr] + D[Rr+1] on its fluid nodes
+            const SpRow& rw = S.row[Rr & (SP_NR - 1)];
+            const V* Ub = S.U[(Rr - 1) & (SP_NRU - 1)];
+            const V* Mb = S.M[Rr & (SP_NRU - 1)];
+            const V* Db = S.D[(Rr + 1) & (SP_NRU - 1)];
+            const int hlF = (int)(rw.hlr & 1u);
+            const int nb = (int)rw.n - hlF - (int)(rw.hlr >> 1);   // body entries
+            R* prow = phi_out + (size_t)rw.jrow * (size_t)nx + (size_t)c0 * NL;
+            for (int e = lane; e < nb; e += 32) {
+              const uint2 mt = S.meta[rw.off + hlF + e];
+              const int c = (int)(mt.x & 0xffffu) - c0;
+              const V v = (Ub[c + 1] + Mb[c + 1]) + Db[c + 1];
+              const unsigned fl = (mt.x >> 16) & 0xfu;
+              R* dst = prow + c * NL;
+              if (fl == (1u << NL) - 1u) store_vec<V>(dst, v);
+              else {
+                R x[NL];
+                L::unpack(v, x);
+#pragma unroll
+                for (int k = 0; k < NL; k++)
+                  if ((fl >> k) & 1u) dst[k] = x[k];
+              }
+            }
+          }
+          Rret++;
+          continue;
+        }
+        if (can_um) {
+          V* Ub = S.U[Rum & (SP_NRU - 1)];
+          V* Db = S.D[Rum & (SP_NRU - 1)];
+          for (int k = lane; k < SP_S + 2; k += 32) { Ub[k] = zero; Db[k] = zero; }
+          __syncwarp();
+          if (lane == 0) st_release(&S.um_ready, Rum);
+          Rum++;
+          continue;
+        }
+        // (c) load the next row if a row slot and ring space are free
+        bool loaded = false;
+        if (Rload < nR && Rload - Rret < SP_NR) {
+          const SpDesc d = dn;
+          const int n = (int)d.hl + (int)d.a + (int)d.hr;
+          const int need = (n + 8) & ~1;
+          int start = -1;
+          if (Rret == Rload) { start = 0; }
+          else {
+            const int tail = S.rstart[Rret & (SP_NR - 1)];
+            if (head >= tail) {
+              if (head + need <= SP_CAP) start = head;
+              else if (need < tail) start = 0;
+            } else if (head + need < tail) start = head;
+          }
+          if (start >= 0) {
+            const int Rr = Rload, slot = Rr & (SP_NR - 1);
+            const int j = grid_row(Rr);
+            const bool contL = d.hl && d.ciL + 1u == d.ci0;
+            const bool contR = d.hr && d.ciR == d.ci0 + d.a;
+            const unsigned runCi = d.ci0 - (contL ? 1u : 0u);
+            const int runLen = (int)d.a + (contL ? 1 : 0) + (contR ? 1 : 0);
+            int off0 = start + 2;
+            int runRing = off0 + ((d.hl && !contL) ? 1 : 0);
+            if ((runRing ^ (int)runCi) & 1) { off0++; runRing++; }
+            if (lane == 0) {
+              SpRow& rw = S.row[slot];
+              rw.off = (uint32_t)off0; rw.ci0 = d.ci0; rw.n = (uint32_t)n; rw.hlr = (uint32_t)d.hl | ((uint32_t)d.hr << 1);
+              rw.bits[0] = d.bits[0]; rw.bits[1] = d.bits[1]; rw.bits[2] = d.bits[2]; rw.bits[3] = d.bits[3];
+              rw.pre = (uint32_t)d.pre[0] | ((uint32_t)d.pre[1] << 8) | ((uint32_t)d.pre[2] << 16) | ((uint32_t)d.pre[3] << 24);
+              rw.jrow = (uint32_t)j; rw.metaL = d.metaL; rw.metaR = d.metaR;
+              S.rstart[slot] = start;
+            }
+            // bulk copies: lanes 0..8 one population plane each, lane 9 the metadata, lane 10 the phi row
+            const unsigned mb = (unsigned)__cvta_generic_to_shared(&S.full[slot]);
+            const unsigned nHalo = ((d.hl && !contL) ? 1u : 0u) + ((d.hr && !contR) ? 1u : 0u);
+            const unsigned mStart = d.ci0 & ~1u, mEnd = (d.ci0 + d.a + 1u) & ~1u;
+            const unsigned metaBytes = d.a ? (mEnd - mStart) * 8u : 0u;
+            const unsigned phiBytes = (unsigned)(seff + 4) * 16u;
+            const unsigned bytes = 9u * 16u * ((unsigned)runLen + nHalo) + metaBytes + phiBytes;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            if (lane == 0) mbar_arrive_tx(mb, bytes);
+            __syncwarp();
+            if (lane < 9) {
+              const char* src = reinterpret_cast<const char*>(Nsrc) + (size_t)cpsB * (unsigned)lane;
+              if (runLen > 0)
+                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[lane][runRing]), src + (size_t)runCi * 16u,
+                         (unsigned)runLen * 16u, mb);
+              if (d.hl && !contL)
+                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[lane][off0]), src + (size_t)d.ciL * 16u, 16u, mb);
+              if (d.hr && !contR)
+                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[lane][off0 + n - 1]), src + (size_t)d.ciR * 16u, 16u, mb);
+            } else if (lane == 9) {
+              if (metaBytes)
+                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.meta[off0 + (int)d.hl - (int)(d.ci0 & 1u)]),
+                         gmeta + mStart, metaBytes, mb);
+            } else if (lane == 10) {
+              // logical groups c0-2 .. c0+seff+1 of the periodic row, cut where they wrap
+              int g = c0 - 2, left = seff + 4, dsti = 0;
+              const R* prow = phi_in + (size_t)j * (size_t)nx;
+              while (left > 0) {
+                int gw = g % ng;
+                if (gw < 0) gw += ng;
+                const int len = min(left, ng - gw);
+                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.phi[slot][dsti]), prow + (size_t)gw * NL, (unsigned)len * 16u, mb);
+                g += len; left -= len; dsti += len;
+              }
+            }
+            head = start + need;
+            Rload++;
+            if (Rload < nR) dn = sdesc[grid_row(Rload)];
+            loaded = true;
+          }
+        }
+        if (!loaded) __nanosleep(100);
+      }
+    } else {
+      // ===================================== consumer warps =====================================
+      int waitedR = -1;   // full[] observed for ring rows <= waitedR
+      auto row_of = [&](int s) -> int {   // processed row R (1 .. TY+2) holding position s: T[R-1] <= s < T[R]
+        int lo = 1, hi = TY + 2;
+        while (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if ((int)S.T[mid] <= s) lo = mid + 1; else hi = mid;
+        }
+        return lo;
+      };
+      // a warp has no claim on the rows before its first pass
+      if (lane == 0) st_release(&S.done[warp], warp < NP ? row_of(max(30 * warp - 1, 0)) - 1 : TY + 2);
+      for (int p = warp; p < NP; p += SP_W) {
+        const int s0 = 30 * p - 1;
+        const int R0 = row_of(max(s0, 0));
+        const int s = s0 + lane;
+        int Rl = R0;
+#pragma unroll
+        for (int k = 0; k < 5; k++)
+          if (R0 + k <= TY + 1 && s >= (int)S.T[R0 + k]) Rl = R0 + k + 1;
+        const bool pos_ok = s >= 0 && s < P;
+        const int e = s - (int)S.T[Rl - 1];
+        const int Rmax = __shfl_sync(FULL, Rl, 31);
+        // rows R0-1 .. Rmax+1 must have landed
+        while (waitedR < Rmax + 1) {
+          waitedR++;
+          mbar_wait((unsigned)__cvta_generic_to_shared(&S.full[waitedR & (SP_NR - 1)]), (unsigned)(waitedR / SP_NR) & 1u);
+        }
+        wait_counter(&S.um_ready, Rmax);
+
+        const SpRow& rw = S.row[Rl & (SP_NR - 1)];
+        const bool active = pos_ok && e < (int)rw.n;
+        const bool outl = active && lane >= 1 && lane <= 30;
+        uint2 mt = make_uint2(0u, 0u);
+        int c = 0;
+        bool body = false;
+        if (active) {
+          if (e == 0 && (rw.hlr & 1u)) { mt = rw.metaL; c = -1; }
+          else if (e == (int)rw.n - 1 && (rw.hlr & 2u)) { mt = rw.metaR; c = seff; }
+          else { mt = S.meta[rw.off + e]; c = (int)(mt.x & 0xffffu) - c0; body = true; }
+        }
+        bool fl[NL];
+        unsigned lk[NL];
+        bool any_fl = false, all_fl = true;
+        unsigned lk_any = 0u;
+#pragma unroll
+        for (int k = 0; k < NL; k++) {
+          fl[k] = active && ((mt.x >> (16 + k)) & 1u);
+          lk[k] = fl[k] ? ((mt.y >> (8 * k)) & 0xffu) : 0u;
+          any_fl |= fl[k]; all_fl &= fl[k]; lk_any |= lk[k];
+        }
+        const bool adjL = active && ((mt.x >> 20) & 1u) && e > 0;
+        const bool adjR = active && ((mt.x >> 21) & 1u) && e + 1 < (int)rw.n;
+
+        V bs[9];
+        V bb = zero;
+        if (active) {
+          const SpRow& ru = S.row[(Rl - 1) & (SP_NR - 1)];
+          const SpRow& rd = S.row[(Rl + 1) & (SP_NR - 1)];
+          unsigned bU, bD;
+          const int eu = (int)ru.off + sp_rank(ru, c, &bU);
+          const int ed = (int)rd.off + sp_rank(rd, c, &bD);
+          const int eo = (int)rw.off + e;
+          // own-position populations of the node's row, and the neighbours' (propagation A16-A17)
+          const V o0 = S.N[0][eo], o1 = S.N[1][eo], o2 = S.N[2][eo], o3 = S.N[3][eo], o4 = S.N[4][eo],
+                  o5 = S.N[5][eo], o6 = S.N[6][eo], o7 = S.N[7][eo], o8 = S.N[8][eo];
+          V nn[9];
+          nn[0] = o0;
+          nn[1] = shift_in_left<V>(o1, reinterpret_cast<const R*>(&S.N[1][eo - 1])[NL - 1]);
+          nn[3] = shift_in_right<V>(o3, reinterpret_cast<const R*>(&S.N[3][eo + 1])[0]);
+          nn[2] = S.N[2][eu];
+          nn[5] = shift_in_left<V>(S.N[5][eu], reinterpret_cast<const R*>(&S.N[5][eu - 1])[NL - 1]);
+          nn[6] = shift_in_right<V>(S.N[6][eu], reinterpret_cast<const R*>(&S.N[6][eu + (int)bU])[0]);
+          nn[4] = S.N[4][ed];
+          nn[7] = shift_in_right<V>(S.N[7][ed], reinterpret_cast<const R*>(&S.N[7][ed + (int)bD])[0]);
+          nn[8] = shift_in_left<V>(S.N[8][ed], reinterpret_cast<const R*>(&S.N[8][ed - 1])[NL - 1]);
+          if (lk_any) {   // half-way bounce-back (R12): the node's own opposite population
+            const V own[9] = {o0, o1, o2, o3, o4, o5, o6, o7, o8};
+#pragma unroll
+            for (int q = 1; q < 9; q++) {
+              R a[NL], o[NL];
+              L::unpack(nn[q], a);
+              L::unpack(own[opp(q)], o);
+#pragma unroll
+              for (int k = 0; k < NL; k++)
+                if ((lk[k] >> (q - 1)) & 1u) a[k] = o[k];
+              nn[q] = L::pack(a);
+            }
+          }
+          // phi stencil (R8): nodes c*NL - 1 .. c*NL + NL of the three rows; row buffers start at group -2
+          const R* pu = reinterpret_cast<const R*>(&S.phi[(Rl - 1) & (SP_NR - 1)][c + 2]);
+          const R* pc = reinterpret_cast<const R*>(&S.phi[Rl & (SP_NR - 1)][c + 2]);
+          const R* pd = reinterpret_cast<const R*>(&S.phi[(Rl + 1) & (SP_NR - 1)][c + 2]);
+          const V pS = *reinterpret_cast<const V*>(pu), pC = *reinterpret_cast<const V*>(pc), pN = *reinterpret_cast<const V*>(pd);
+          const V ph[9] = {pC, shift_in_right<V>(pC, pc[NL]), pN, shift_in_left<V>(pC, pc[-1]), pS,
+                           shift_in_right<V>(pN, pd[NL]), shift_in_left<V>(pN, pd[-1]),
+                           shift_in_left<V>(pS, pu[-1]), shift_in_right<V>(pS, pu[NL])};
+          V ns[9];
+          collide_lane<V>(C, nn, ph, fl, all_fl, ns, bs);
+          if (outl && body && Rl >= 2 && Rl <= TY + 1) {
+            const unsigned ci = rw.ci0 + (unsigned)(e - (int)(rw.hlr & 1u));
+            char* dst = reinterpret_cast<char*>(Ndst) + (size_t)ci * 16u;
+#pragma unroll
+            for (int q = 0; q < 9; q++) store_vec<V>(dst + (size_t)cpsB * (unsigned)q, ns[q]);
+            if (WRITE_B) {
+              char* dstB = reinterpret_cast<char*>(Bdst + ((size_t)rw.jrow * (size_t)nx + (size_t)(c0 + c) * NL));
+#pragma unroll
+              for (int q = 0; q < 9; q++) *reinterpret_cast<V*>(dstB + (size_t)psBd * (unsigned)q) = bs[q];
+            }
+          }
+          if (lk_any) {   // link q hands the node its own B_opp(q)* back
+            R b[NL];
+#pragma unroll
+            for (int k = 0; k < NL; k++) b[k] = R(0);
+#pragma unroll
+            for (int q = 1; q < 9; q++) {
+              R o[NL];
+              L::unpack(bs[opp(q)], o);
+#pragma unroll
+              for (int k = 0; k < NL; k++)
+                if ((lk[k] >> (q - 1)) & 1u) b[k] += o[k];
+            }
+            bb = L::pack(b);
+          }
+        } else {
+#pragma unroll
+          for (int q = 0; q < 9; q++) bs[q] = zero;
+        }
+        // contributions of this group's row to phi(t+1) of the rows above (U), at (M) and below (D): the B*
+        // that move in x cross to the x-adjacent lane by shuffle; a neighbour group without a fluid node has
+        // no lane, so the node next to it gets the spill by a direct store
+        const R z = R(0);
+        const R l1 = __shfl_up_sync(FULL, last_of<V>(bs[1]), 1), l5 = __shfl_up_sync(FULL, last_of<V>(bs[5]), 1),
+                l8 = __shfl_up_sync(FULL, last_of<V>(bs[8]), 1);
+        const R r3 = __shfl_down_sync(FULL, first_of<V>(bs[3]), 1), r6 = __shfl_down_sync(FULL, first_of<V>(bs[6]), 1),
+                r7 = __shfl_down_sync(FULL, first_of<V>(bs[7]), 1);
+        if (outl) {
+          const int ub = Rl & (SP_NRU - 1);
+          if (body) {
+            const V mid = (bs[0] + shift_in_left<V>(bs[1], adjL ? l1 : z)) + shift_in_right<V>(bs[3], adjR ? r3 : z);
+            const V upw = (bs[2] + shift_in_left<V>(bs[5], adjL ? l5 : z)) + shift_in_right<V>(bs[6], adjR ? r6 : z);
+            const V dwn = (bs[4] + shift_in_right<V>(bs[7], adjR ? r7 : z)) + shift_in_left<V>(bs[8], adjL ? l8 : z);
+            S.U[ub][c + 1] = upw;
+            S.M[ub][c + 1] = mid + bb;
+            S.D[ub][c + 1] = dwn;
+          }
+          // spills into the columns of a body group that has no lane in this row
+          if (!adjR && c + 1 >= 0 && c + 1 < seff && !(((rw.bits[(c + 2) >> 5]) >> ((c + 2) & 31)) & 1u)) {
+            reinterpret_cast<R*>(&S.U[ub][c + 2])[0] = last_of<V>(bs[5]);
+            reinterpret_cast<R*>(&S.D[ub][c + 2])[0] = last_of<V>(bs[8]);
+          }
+          if (!adjL && c - 1 >= 0 && c - 1 < seff && !(((rw.bits[c >> 5]) >> (c & 31)) & 1u)) {
+            reinterpret_cast<R*>(&S.U[ub][c])[NL - 1] = first_of<V>(bs[6]);
+            reinterpret_cast<R*>(&S.D[ub][c])[NL - 1] = first_of<V>(bs[7]);
+          }
+        }
+        // done with every row before the first row of my next pass
+        __syncwarp();
+        if (lane == 0) {
+          const int pn = p + SP_W;
+          const int dn_row = pn < NP ? row_of(30 * pn - 1) - 1 : TY + 2;
+          st_release(&S.done[warp], dn_row);
+        }
+      }
+    }
+    __syncthreads();
+    if (tid == 32)
+      for (int k = 0; k < SP_NR; k++) mbar_inval((unsigned)__cvta_generic_to_shared(&S.full[k]));
+  }
+}
+
+// ---- one-time builders (lbm_create) ----
+// per compact group: column, fluid bits, x-neighbour groups active, link bytes
+__global__ void __launch_bounds__(256) k_sp_meta(const uint8_t* __restrict__ cls, const uint8_t* __restrict__ links,
+                                                 const uint2* __restrict__ ptab, int nx, int ny, int nw, int G,
+                                                 uint2* __restrict__ gmeta) {
+  const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
+  const int ng = nx / G;
+  if (t >= (long long)ny * ng) return;
+  const int r = (int)(t / ng), p = (int)(t % ng);
+  const uint2* prow = ptab + (size_t)r * nw;
+  auto act = [&](int g) -> unsigned { return (prow[g >> 5].x >> (g & 31)) & 1u; };
+  if (!act(p)) return;
+  const uint2 tb = prow[p >> 5];
+  const size_t ci = (size_t)tb.y + (size_t)__popc(tb.x & ((1u << (p & 31)) - 1u));
+  const size_t k = (size_t)r * nx + (size_t)G * p;
+  unsigned fl = 0, lk = 0;
+  for (int c = 0; c < G; c++)
+    if (cls[k + c] < 2) { fl |= 1u << c; lk |= (unsigned)links[k + c] << (8 * c); }
+  const unsigned aL = act(p == 0 ? ng - 1 : p - 1), aR = act(p == ng - 1 ? 0 : p + 1);
+  gmeta[ci] = make_uint2((unsigned)p | (fl << 16) | (aL << 20) | (aR << 21), lk);
+}
+
+__global__ void __launch_bounds__(128) k_sp_desc(const uint2* __restrict__ ptab, const uint2* __restrict__ gmeta, int nx,
+                                                 int ny, int nw, int G, int nstrips, SpDesc* __restrict__ desc,
+                                                 uint16_t* __restrict__ cnt) {
+  const long long t = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (t >= (long long)nstrips * ny) return;
+  const int strip = (int)(t / ny), r = (int)(t % ny);
+  const int ng = nx / G;
+  const int c0 = strip * SP_S, seff = min(SP_S, ng - c0);
+  const uint2* prow = ptab + (size_t)r * nw;
+  auto wrapg = [&](int g) -> int { g %= ng; return g < 0 ? g + ng : g; };
+  auto act = [&](int g) -> unsigned { return (prow[g >> 5].x >> (g & 31)) & 1u; };
+  auto cidx = [&](int g) -> unsigned {
+    const uint2 tb = prow[g >> 5];
+    return tb.y + (unsigned)__popc(tb.x & ((1u << (g & 31)) - 1u));
+  };
+  SpDesc d;
+  memset(&d, 0, sizeof d);
+  for (int c = -1; c <= seff; c++)
+    if (act(wrapg(c0 + c))) d.bits[(c + 1) >> 5] |= 1u << ((c + 1) & 31);
+  unsigned run = 0;
+  for (int w = 0; w < 4; w++) { d.pre[w] = (uint8_t)run; run += (unsigned)__popc(d.bits[w]); }
+  d.hl = (uint8_t)(d.bits[0] & 1u);
+  d.hr = (uint8_t)((d.bits[(seff + 1) >> 5] >> ((seff + 1) & 31)) & 1u);
+  d.a = (uint16_t)(run - d.hl - d.hr);
+  d.ci0 = cidx(c0);
+  d.ciL = cidx(wrapg(c0 - 1));
+  d.ciR = cidx(wrapg(c0 + seff));
+  if (d.hl) d.metaL = gmeta[d.ciL];
+  if (d.hr) d.metaR = gmeta[d.ciR];
+  desc[t] = d;
+  cnt[t] = (uint16_t)run;
+}
+
+}  // namespace lbm

@@ -13,9 +13,9 @@ from paper_2605_30878_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-BASELINE, FUSED, WARP, PAIR, PACK = 1, 2, 3, 4, 5
+BASELINE, FUSED, WARP, PAIR, PACK, SPARSE = 1, 2, 3, 4, 5, 6
 SCHEDULES = [pytest.param(BASELINE, id="baseline"), pytest.param(FUSED, id="fused"), pytest.param(WARP, id="warp"),
-             pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack")]
+             pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack"), pytest.param(SPARSE, id="sparse")]
 
 
 # ---- local update of single nodes ---------------------------------------------------------------
@@ -282,7 +282,7 @@ def test_config3_density_ratio_1000_short():
 
 
 @pytest.mark.parametrize("sched", [pytest.param(FUSED, id="fused"), pytest.param(WARP, id="warp"), pytest.param(PAIR, id="pair"),
-                                   pytest.param(PACK, id="pack")])
+                                   pytest.param(PACK, id="pack"), pytest.param(SPARSE, id="sparse")])
 def test_schedules_agree_and_get_is_idempotent(sched):
     w = wl.config5(seed=3, n=256)
     a, _ = make_pair(w, schedule=BASELINE)
@@ -500,7 +500,7 @@ def test_layout_copy_helper_leaves_the_state_alone():
         assert np.array_equal(b[k], c[k]), k            # same as a run without the helper, bit for bit
 
 
-@pytest.mark.parametrize("schedule", [pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack")])
+@pytest.mark.parametrize("schedule", [pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack"), pytest.param(SPARSE, id="sparse")])
 @pytest.mark.parametrize("shape,frac", [((7, 4), 0.2), ((9, 12), 0.3), ((33, 36), 0.3), ((50, 100), 0.25),
                                         ((61, 244), 0.3), ((40, 126), 0.3)])
 def test_random_masks_ragged_fp32(schedule, shape, frac):
