@@ -78,7 +78,7 @@ struct lbm_ctx {
   void* Nc[2];
   // SPARSE schedule: per (strip, row) descriptors, per-group metadata, the marches of every CTA
   int sparse;
-  int sp_nstrips, sp_ncta, sp_nmarch;
+  int sp_nstrips, sp_ncta, sp_nmarch, sp_sw;
   SpDesc* sp_desc;
   uint16_t* sp_cnt;
   uint2* sp_meta;
@@ -414,7 +414,7 @@ bool launch_sparse_v(lbm_ctx* c, const Consts<R>& C, const R* Ns, R* Nd, R* Bd, 
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
   const unsigned cpsB = (unsigned)(c->cps * 16);
   kern<<<c->sp_ncta, SP_THREADS, smem, c->st>>>(C, Ns, Nd, Bd, pi, po, c->sp_desc, c->sp_cnt, c->sp_meta, c->sp_march,
-                                               c->sp_first, cpsB);
+                                               c->sp_first, cpsB, c->sp_sw);
   return true;
 }
 bool launch_fused_sparse(lbm_ctx* c, const Consts<double>& C, const double* Ns, double* Nd, double* Bd, const double* pi,
@@ -431,7 +431,7 @@ bool launch_fused_sparse(lbm_ctx* c, const Consts<float>& C, const float* Ns, fl
 void sp_partition(const uint16_t* cnt, int nstrips, int ny, int ncta_max, std::vector<SpMarch>& marches,
                   std::vector<int>& first) {
   double total = 0.0;
-  auto weight = [&](int s, int r) { return (double)std::max<int>(cnt[(size_t)s * ny + r], SP_MINPOS) + 4.0; };
+  auto weight = [&](int s, int r) { return (double)std::max<int>(cnt[(size_t)s * ny + r], SP_MINPOS) + 12.0; };
   for (int s = 0; s < nstrips; s++)
     for (int r = 0; r < ny; r++) total += weight(s, r);
   // a CTA should have at least ~64 rows of a full strip to amortise its 4 halo rows
@@ -688,7 +688,9 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     const size_t nsr = (size_t)nstrips * prm->ny;
     k_sp_meta<<<(unsigned)(((long long)prm->ny * ng + 255) / 256), 256, 0, c->st>>>(c->cls, c->links, c->ptab, prm->nx, prm->ny,
                                                                                  c->nw, G, c->sp_meta);
-    k_sp_desc<<<(unsigned)((nsr + 127) / 128), 128, 0, c->st>>>(c->ptab, c->sp_meta, prm->nx, prm->ny, c->nw, G, nstrips,
+    const int sw = (ng + nstrips - 1) / nstrips;   // strips of equal width (<= SP_S groups)
+    c->sp_sw = sw;
+    k_sp_desc<<<(unsigned)((nsr + 127) / 128), 128, 0, c->st>>>(c->ptab, c->sp_meta, prm->nx, prm->ny, c->nw, G, nstrips, sw,
                                                                c->sp_desc, c->sp_cnt);
     CKC(cudaGetLastError());
     std::vector<uint16_t> h_cnt(nsr);

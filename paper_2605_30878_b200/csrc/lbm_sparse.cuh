@@ -31,17 +31,19 @@ namespace lbm {
 #define LBM_SP_WARPS 12
 #endif
 #ifndef LBM_SP_CAP
-#define LBM_SP_CAP 832
+#define LBM_SP_CAP 928
 #endif
 constexpr int SP_S = 126;                 // body groups of a strip; S + 2 halo groups = 128 mask bits
 constexpr int SP_W = LBM_SP_WARPS;        // consumer warps (+ 1 producer warp)
 constexpr int SP_NR = 16;                 // row slots (phi rows, row info, full barriers)
-constexpr int SP_NRU = 8;                 // row slots of the partial-sum buffers
 constexpr int SP_CAP = LBM_SP_CAP;        // entries of the population ring
 constexpr int SP_TYMAX = 512;             // rows of a march
 constexpr int SP_MINPOS = 8;              // a row takes at least this many positions of the pass sequence, so
                                           // that a pass of 32 positions spans at most 5 rows
-constexpr int SP_THREADS = 32 * (SP_W + 1);
+constexpr int SP_K = 2;                   // loader warps and finaliser warps; helper k serves rows R = k (mod K)
+constexpr int SP_CAPK = SP_CAP / SP_K;    // every loader fills its own part of the ring
+constexpr int SP_THREADS = 32 * (SP_W + 2 * SP_K);
+static_assert(SP_NR % SP_K == 0 && SP_CAP % (2 * SP_K) == 0, "helper classes");
 
 // per (strip, row) descriptor, built once by k_sp_desc
 struct __align__(16) SpDesc {
@@ -76,16 +78,14 @@ struct SpSmem {
   V N[9][SP_CAP];
   uint2 meta[SP_CAP];
   V phi[SP_NR][SP_S + 4];
-  V U[SP_NRU][SP_S + 2];
-  V M[SP_NRU][SP_S + 2];
-  V D[SP_NRU][SP_S + 2];
+  V A[3][SP_CAP];       // per entry: what the rows above / at / below contribute to its phi(t+1)
   SpRow row[SP_NR];
   uint32_t T[SP_TYMAX + 4];
   unsigned long long full[SP_NR];
   int rstart[SP_NR];
   int done[32];
-  int um_ready;
-  int pad[3];
+  int ret_row[SP_K];    // class k: rows R = k (mod K) below ret_row[k] are retired
+  int pad[4 - SP_K % 4];
 };
 
 // ---- mbarrier / bulk-copy / ordered shared-memory access ----
@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
                    typename LaneOf<V>::R* __restrict__ Ndst, typename LaneOf<V>::R* __restrict__ Bdst,
                    const typename LaneOf<V>::R* __restrict__ phi_in, typename LaneOf<V>::R* __restrict__ phi_out,
                    const SpDesc* __restrict__ desc, const uint16_t* __restrict__ cnt, const uint2* __restrict__ gmeta,
-                   const SpMarch* __restrict__ marches, const int* __restrict__ cta_first, unsigned cpsB) {
+                   const SpMarch* __restrict__ marches, const int* __restrict__ cta_first, unsigned cpsB, int sw) {
   using L = LaneOf<V>;
   using R = typename L::R;
   constexpr int NL = L::NL;
@@ -204,8 +204,8 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
 
   for (int mi = cta_first[blockIdx.x]; mi < cta_first[blockIdx.x + 1]; mi++) {
     const SpMarch mar = marches[mi];
-    const int c0 = mar.strip * SP_S;                           // first body group of the strip
-    const int seff = min(SP_S, ng - c0);                       // body groups of this strip
+    const int c0 = mar.strip * sw;                             // first body group of the strip (sw <= SP_S groups wide)
+    const int seff = min(sw, ng - c0);                         // body groups of this strip
     const int TY = mar.rows;
     const int nR = TY + 4;                                     // ring rows R = 0 .. TY+3 <-> grid rows j0-2 ..
     const SpDesc* sdesc = desc + (size_t)mar.strip * ny;
@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
     }
     if (tid == 32) {
       for (int k = 0; k < SP_NR; k++) mbar_init((unsigned)__cvta_generic_to_shared(&S.full[k]), 1);
-      S.um_ready = 0;
+      for (int k = 0; k < SP_K; k++) S.ret_row[k] = k;
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < 32) S.done[tid] = 0;
@@ -245,152 +245,160 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
     const int P = (int)S.T[TY + 2];
     const int NP = (P + 29) / 30;
 
-    if (warp == SP_W) {
-      // =============================== producer / finaliser warp ===============================
-      int Rload = 0, Rret = 0, Rum = 1, head = 0;
-      SpDesc dn = sdesc[grid_row(0)];
-      while (Rret < nR) {
-        // (a) retire the oldest row if every consumer is past it
-        int mind = 0x7fffffff;
-        {
-          const int v = lane < SP_W ? ld_acquire(&S.done[lane]) : 0x7fffffff;
-          mind = v;
+    if (warp >= SP_W && warp < SP_W + SP_K) {
+      // ===================== loader warp k: rows R = k (mod K) -> its part of the ring (TMA) =====================
+      const int kc = warp - SP_W;
+      const int rbase = kc * SP_CAPK;
+      int head = 0, Rret = kc;
+      int j = grid_row(kc);
+      int jn = j + SP_K >= ny ? j + SP_K - ny : j + SP_K;
+      SpDesc dn = sdesc[j];
+      for (int Rload = kc; Rload < nR; Rload += SP_K) {
+        const SpDesc d = dn;
+        const int jcur = j;
+        j = jn;
+        jn = j + SP_K >= ny ? j + SP_K - ny : j + SP_K;
+        if (Rload + SP_K < nR) dn = sdesc[j];
+        const int n = (int)d.hl + (int)d.a + (int)d.hr;
+        const int need = (n + 8) & ~1;
+        // wait for a row slot and for ring space (the rows of a class are retired in order by its finaliser)
+        int start = -1;
+        long long t0 = 0;
+        for (;;) {
+          if (Rload - Rret < SP_NR) {
+            if (Rret == Rload) { start = 0; }
+            else {
+              const int tail = S.rstart[Rret & (SP_NR - 1)];
+              if (head >= tail) {
+                if (head + need <= SP_CAPK) start = head;
+                else if (need < tail) start = 0;
+              } else if (head + need < tail) start = head;
+            }
+          }
+          if (start >= 0) break;
+          const int r = ld_acquire(&S.ret_row[kc]);
+          if (r == Rret) {
+            __nanosleep(32);
+            if (t0 == 0) t0 = clock64();
+            else if (clock64() - t0 > 8000000000LL) __trap();
+          }
+          Rret = r;
+        }
+        const int slot = Rload & (SP_NR - 1);
+        const bool contL = d.hl && d.ciL + 1u == d.ci0;
+        const bool contR = d.hr && d.ciR == d.ci0 + d.a;
+        const unsigned runCi = d.ci0 - (contL ? 1u : 0u);
+        const int runLen = (int)d.a + (contL ? 1 : 0) + (contR ? 1 : 0);
+        int off0 = rbase + start + 2;
+        int runRing = off0 + ((d.hl && !contL) ? 1 : 0);
+        if ((runRing ^ (int)runCi) & 1) { off0++; runRing++; }
+        head = start + need;
+        // nobody has written the row's phi(t+1) contributions yet: the sums from above and below start at zero
+        for (int e = lane; e < n; e += 32) { S.A[0][off0 + e] = zero; S.A[2][off0 + e] = zero; }
+        __syncwarp();
+        if (lane == 0) {
+          SpRow& rw = S.row[slot];
+          rw.off = (uint32_t)off0; rw.ci0 = d.ci0; rw.n = (uint32_t)n; rw.hlr = (uint32_t)d.hl | ((uint32_t)d.hr << 1);
+          rw.bits[0] = d.bits[0]; rw.bits[1] = d.bits[1]; rw.bits[2] = d.bits[2]; rw.bits[3] = d.bits[3];
+          rw.pre = (uint32_t)d.pre[0] | ((uint32_t)d.pre[1] << 8) | ((uint32_t)d.pre[2] << 16) | ((uint32_t)d.pre[3] << 24);
+          rw.jrow = (uint32_t)jcur; rw.metaL = d.metaL; rw.metaR = d.metaR;
+          S.rstart[slot] = start;
+          // one elected lane issues every bulk copy of the row (uniform datapath, no per-lane serialisation)
+          const unsigned mb = (unsigned)__cvta_generic_to_shared(&S.full[slot]);
+          const bool wl = d.hl && !contL, wr = d.hr && !contR;
+          const unsigned mStart = d.ci0 & ~1u, mEnd = (d.ci0 + d.a + 1u) & ~1u;
+          const unsigned metaBytes = d.a ? (mEnd - mStart) * 8u : 0u;
+          const unsigned phiBytes = (unsigned)(seff + 4) * 16u;
+          const unsigned bytes = 9u * 16u * ((unsigned)runLen + (wl ? 1u : 0u) + (wr ? 1u : 0u)) + metaBytes + phiBytes;
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          mbar_arrive_tx(mb, bytes);
+          const char* src = reinterpret_cast<const char*>(Nsrc);
+          const unsigned dN = (unsigned)__cvta_generic_to_shared(&S.N[0][0]);
+          if (runLen > 0) {
 #pragma unroll
-          for (int d = 16; d >= 1; d >>= 1) mind = min(mind, __shfl_xor_sync(FULL, mind, d));
-        }
-        const bool can_retire = Rret < Rload && mind >= min(Rret + 1, TY + 2);
-        // (b) partial-sum buffers of processed row Rum: free once finalise(Rum - NRU + 1) is done
-        const bool can_um = Rum <= TY + 2 && (Rum - SP_NRU < 1 || Rret >= Rum - SP_NRU + 2);
-        if (can_retire) {
-          const int Rr = Rret;
-          if (Rr >= 2 && Rr <= TY + 1) {   // phi(t+1) of row Rr = U[Rr-1] + M[Rr] + D[Rr+1] on its fluid nodes
-            const SpRow& rw = S.row[Rr & (SP_NR - 1)];
-            const V* Ub = S.U[(Rr - 1) & (SP_NRU - 1)];
-            const V* Mb = S.M[Rr & (SP_NRU - 1)];
-            const V* Db = S.D[(Rr + 1) & (SP_NRU - 1)];
-            const int hlF = (int)(rw.hlr & 1u);
-            const int nb = (int)rw.n - hlF - (int)(rw.hlr >> 1);   // body entries
-            R* prow = phi_out + (size_t)rw.jrow * (size_t)nx + (size_t)c0 * NL;
-            for (int e = lane; e < nb; e += 32) {
-              const uint2 mt = S.meta[rw.off + hlF + e];
-              const int c = (int)(mt.x & 0xffffu) - c0;
-              const V v = (Ub[c + 1] + Mb[c + 1]) + Db[c + 1];
-              const unsigned fl = (mt.x >> 16) & 0xfu;
-              R* dst = prow + c * NL;
-              if (fl == (1u << NL) - 1u) store_vec<V>(dst, v);
-              else {
-                R x[NL];
-                L::unpack(v, x);
+            for (int q = 0; q < 9; q++)
+              bulk_g2s(dN + (unsigned)(q * SP_CAP + runRing) * 16u, src + (size_t)cpsB * (unsigned)q + (size_t)runCi * 16u,
+                       (unsigned)runLen * 16u, mb);
+          }
+          if (wl) {
 #pragma unroll
-                for (int k = 0; k < NL; k++)
-                  if ((fl >> k) & 1u) dst[k] = x[k];
-              }
-            }
+            for (int q = 0; q < 9; q++)
+              bulk_g2s(dN + (unsigned)(q * SP_CAP + off0) * 16u, src + (size_t)cpsB * (unsigned)q + (size_t)d.ciL * 16u, 16u, mb);
           }
-          Rret++;
-          continue;
-        }
-        if (can_um) {
-          V* Ub = S.U[Rum & (SP_NRU - 1)];
-          V* Db = S.D[Rum & (SP_NRU - 1)];
-          for (int k = lane; k < SP_S + 2; k += 32) { Ub[k] = zero; Db[k] = zero; }
-          __syncwarp();
-          if (lane == 0) st_release(&S.um_ready, Rum);
-          Rum++;
-          continue;
-        }
-        // (c) load the next row if a row slot and ring space are free
-        bool loaded = false;
-        if (Rload < nR && Rload - Rret < SP_NR) {
-          const SpDesc d = dn;
-          const int n = (int)d.hl + (int)d.a + (int)d.hr;
-          const int need = (n + 8) & ~1;
-          int start = -1;
-          if (Rret == Rload) { start = 0; }
-          else {
-            const int tail = S.rstart[Rret & (SP_NR - 1)];
-            if (head >= tail) {
-              if (head + need <= SP_CAP) start = head;
-              else if (need < tail) start = 0;
-            } else if (head + need < tail) start = head;
+          if (wr) {
+#pragma unroll
+            for (int q = 0; q < 9; q++)
+              bulk_g2s(dN + (unsigned)(q * SP_CAP + off0 + n - 1) * 16u, src + (size_t)cpsB * (unsigned)q + (size_t)d.ciR * 16u, 16u, mb);
           }
-          if (start >= 0) {
-            const int Rr = Rload, slot = Rr & (SP_NR - 1);
-            const int j = grid_row(Rr);
-            const bool contL = d.hl && d.ciL + 1u == d.ci0;
-            const bool contR = d.hr && d.ciR == d.ci0 + d.a;
-            const unsigned runCi = d.ci0 - (contL ? 1u : 0u);
-            const int runLen = (int)d.a + (contL ? 1 : 0) + (contR ? 1 : 0);
-            int off0 = start + 2;
-            int runRing = off0 + ((d.hl && !contL) ? 1 : 0);
-            if ((runRing ^ (int)runCi) & 1) { off0++; runRing++; }
-            if (lane == 0) {
-              SpRow& rw = S.row[slot];
-              rw.off = (uint32_t)off0; rw.ci0 = d.ci0; rw.n = (uint32_t)n; rw.hlr = (uint32_t)d.hl | ((uint32_t)d.hr << 1);
-              rw.bits[0] = d.bits[0]; rw.bits[1] = d.bits[1]; rw.bits[2] = d.bits[2]; rw.bits[3] = d.bits[3];
-              rw.pre = (uint32_t)d.pre[0] | ((uint32_t)d.pre[1] << 8) | ((uint32_t)d.pre[2] << 16) | ((uint32_t)d.pre[3] << 24);
-              rw.jrow = (uint32_t)j; rw.metaL = d.metaL; rw.metaR = d.metaR;
-              S.rstart[slot] = start;
-            }
-            // bulk copies: lanes 0..8 one population plane each, lane 9 the metadata, lane 10 the phi row
-            const unsigned mb = (unsigned)__cvta_generic_to_shared(&S.full[slot]);
-            const unsigned nHalo = ((d.hl && !contL) ? 1u : 0u) + ((d.hr && !contR) ? 1u : 0u);
-            const unsigned mStart = d.ci0 & ~1u, mEnd = (d.ci0 + d.a + 1u) & ~1u;
-            const unsigned metaBytes = d.a ? (mEnd - mStart) * 8u : 0u;
-            const unsigned phiBytes = (unsigned)(seff + 4) * 16u;
-            const unsigned bytes = 9u * 16u * ((unsigned)runLen + nHalo) + metaBytes + phiBytes;
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            if (lane == 0) mbar_arrive_tx(mb, bytes);
-            __syncwarp();
-            if (lane < 9) {
-              const char* src = reinterpret_cast<const char*>(Nsrc) + (size_t)cpsB * (unsigned)lane;
-              if (runLen > 0)
-                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[lane][runRing]), src + (size_t)runCi * 16u,
-                         (unsigned)runLen * 16u, mb);
-              if (d.hl && !contL)
-                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[lane][off0]), src + (size_t)d.ciL * 16u, 16u, mb);
-              if (d.hr && !contR)
-                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[lane][off0 + n - 1]), src + (size_t)d.ciR * 16u, 16u, mb);
-            } else if (lane == 9) {
-              if (metaBytes)
-                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.meta[off0 + (int)d.hl - (int)(d.ci0 & 1u)]),
-                         gmeta + mStart, metaBytes, mb);
-            } else if (lane == 10) {
-              // logical groups c0-2 .. c0+seff+1 of the periodic row, cut where they wrap
-              int g = c0 - 2, left = seff + 4, dsti = 0;
-              const R* prow = phi_in + (size_t)j * (size_t)nx;
-              while (left > 0) {
-                int gw = g % ng;
-                if (gw < 0) gw += ng;
-                const int len = min(left, ng - gw);
-                bulk_g2s((unsigned)__cvta_generic_to_shared(&S.phi[slot][dsti]), prow + (size_t)gw * NL, (unsigned)len * 16u, mb);
-                g += len; left -= len; dsti += len;
-              }
-            }
-            head = start + need;
-            Rload++;
-            if (Rload < nR) dn = sdesc[grid_row(Rload)];
-            loaded = true;
+          if (metaBytes)
+            bulk_g2s((unsigned)__cvta_generic_to_shared(&S.meta[off0 + (int)d.hl - (int)(d.ci0 & 1u)]), gmeta + mStart, metaBytes, mb);
+          // phi: logical groups c0-2 .. c0+seff+1 of the periodic row, cut where they wrap
+          int g = c0 - 2, left = seff + 4, dsti = 0;
+          const R* prow = phi_in + (size_t)jcur * (size_t)nx;
+          while (left > 0) {
+            int gw = g % ng;
+            if (gw < 0) gw += ng;
+            const int len = min(left, ng - gw);
+            bulk_g2s((unsigned)__cvta_generic_to_shared(&S.phi[slot][dsti]), prow + (size_t)gw * NL, (unsigned)len * 16u, mb);
+            g += len; left -= len; dsti += len;
           }
         }
-        if (!loaded) __nanosleep(100);
+        __syncwarp();
+      }
+    } else if (warp >= SP_W + SP_K) {
+      // ==== finaliser warp k: retires the rows R = k (mod K) in order, stores phi(t+1), recycles the sum buffers ====
+      const int kc = warp - SP_W - SP_K;
+      for (int Rret = kc; Rret < nR; Rret += SP_K) {
+        const int want = min(Rret + 1, TY + 2);
+        long long t0 = 0;
+        for (;;) {   // every consumer past row Rret + 1
+          int mind = lane < SP_W ? ld_acquire(&S.done[lane]) : 0x7fffffff;
+#pragma unroll
+          for (int dd = 16; dd >= 1; dd >>= 1) mind = min(mind, __shfl_xor_sync(FULL, mind, dd));
+          if (mind >= want) break;
+          __nanosleep(32);
+          if (t0 == 0) t0 = clock64();
+          else if (clock64() - t0 > 8000000000LL) __trap();
+        }
+        if (Rret >= 2 && Rret <= TY + 1) {   // phi(t+1) of the row: the three partial sums of its entries, on fluid nodes
+          const SpRow& rw = S.row[Rret & (SP_NR - 1)];
+          const int hlF = (int)(rw.hlr & 1u);
+          const int nb = (int)rw.n - hlF - (int)(rw.hlr >> 1);   // body entries
+          R* prow = phi_out + (size_t)rw.jrow * (size_t)nx + (size_t)c0 * NL;
+          const int x0 = (int)rw.off + hlF;
+          for (int e = lane; e < nb; e += 32) {
+            const uint2 mt = S.meta[x0 + e];
+            const int c = (int)(mt.x & 0xffffu) - c0;
+            const V v = (S.A[0][x0 + e] + S.A[1][x0 + e]) + S.A[2][x0 + e];
+            const unsigned fl = (mt.x >> 16) & 0xfu;
+            R* dst = prow + c * NL;
+            if (fl == (1u << NL) - 1u) store_vec<V>(dst, v);
+            else {
+              R x[NL];
+              L::unpack(v, x);
+#pragma unroll
+              for (int k = 0; k < NL; k++)
+                if ((fl >> k) & 1u) dst[k] = x[k];
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) st_release(&S.ret_row[kc], Rret + SP_K);
       }
     } else {
       // ===================================== consumer warps =====================================
       int waitedR = -1;   // full[] observed for ring rows <= waitedR
-      auto row_of = [&](int s) -> int {   // processed row R (1 .. TY+2) holding position s: T[R-1] <= s < T[R]
-        int lo = 1, hi = TY + 2;
-        while (lo < hi) {
-          const int mid = (lo + hi) >> 1;
-          if ((int)S.T[mid] <= s) lo = mid + 1; else hi = mid;
-        }
-        return lo;
+      auto row_scan = [&](int from, int s) -> int {   // processed row R >= from holding position s: T[R-1] <= s < T[R]
+        int r = from;
+        while ((int)S.T[r] <= s) r++;
+        return r;
       };
       // a warp has no claim on the rows before its first pass
-      if (lane == 0) st_release(&S.done[warp], warp < NP ? row_of(max(30 * warp - 1, 0)) - 1 : TY + 2);
+      int Rnext = warp < NP ? row_scan(1, max(30 * warp - 1, 0)) : TY + 3;
+      if (lane == 0) st_release(&S.done[warp], Rnext - 1);
       for (int p = warp; p < NP; p += SP_W) {
         const int s0 = 30 * p - 1;
-        const int R0 = row_of(max(s0, 0));
+        const int R0 = Rnext;
         const int s = s0 + lane;
         int Rl = R0;
 #pragma unroll
@@ -404,8 +412,6 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
           waitedR++;
           mbar_wait((unsigned)__cvta_generic_to_shared(&S.full[waitedR & (SP_NR - 1)]), (unsigned)(waitedR / SP_NR) & 1u);
         }
-        wait_counter(&S.um_ready, Rmax);
-
         const SpRow& rw = S.row[Rl & (SP_NR - 1)];
         const bool active = pos_ok && e < (int)rw.n;
         const bool outl = active && lane >= 1 && lane <= 30;
@@ -432,13 +438,23 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
 
         V bs[9];
         V bb = zero;
+        int eu = 0, ed = 0, eo = 0;          // ring entries of group c in the rows above / below, and of the lane's own group
+        unsigned bU = 0, bD = 0;             // group c holds a fluid node in the row above / below
+        unsigned nbU = 0, nbD = 0;           // bit 0 / 1: group c-1 / c+1 holds a fluid node in the row above (nbU) / below (nbD)
         if (active) {
           const SpRow& ru = S.row[(Rl - 1) & (SP_NR - 1)];
           const SpRow& rd = S.row[(Rl + 1) & (SP_NR - 1)];
-          unsigned bU, bD;
-          const int eu = (int)ru.off + sp_rank(ru, c, &bU);
-          const int ed = (int)rd.off + sp_rank(rd, c, &bD);
-          const int eo = (int)rw.off + e;
+          eu = (int)ru.off + sp_rank(ru, c, &bU);
+          ed = (int)rd.off + sp_rank(rd, c, &bD);
+          eo = (int)rw.off + e;
+          if (c >= 1) {
+            nbU |= (ru.bits[c >> 5] >> (c & 31)) & 1u;
+            nbD |= (rd.bits[c >> 5] >> (c & 31)) & 1u;
+          }
+          if (c + 1 < seff) {
+            nbU |= ((ru.bits[(c + 2) >> 5] >> ((c + 2) & 31)) & 1u) << 1;
+            nbD |= ((rd.bits[(c + 2) >> 5] >> ((c + 2) & 31)) & 1u) << 1;
+          }
           // own-position populations of the node's row, and the neighbours' (propagation A16-A17)
           const V o0 = S.N[0][eo], o1 = S.N[1][eo], o2 = S.N[2][eo], o3 = S.N[3][eo], o4 = S.N[4][eo],
                   o5 = S.N[5][eo], o6 = S.N[6][eo], o7 = S.N[7][eo], o8 = S.N[8][eo];
@@ -513,32 +529,29 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
         const R r3 = __shfl_down_sync(FULL, first_of<V>(bs[3]), 1), r6 = __shfl_down_sync(FULL, first_of<V>(bs[6]), 1),
                 r7 = __shfl_down_sync(FULL, first_of<V>(bs[7]), 1);
         if (outl) {
-          const int ub = Rl & (SP_NRU - 1);
           if (body) {
             const V mid = (bs[0] + shift_in_left<V>(bs[1], adjL ? l1 : z)) + shift_in_right<V>(bs[3], adjR ? r3 : z);
             const V upw = (bs[2] + shift_in_left<V>(bs[5], adjL ? l5 : z)) + shift_in_right<V>(bs[6], adjR ? r6 : z);
             const V dwn = (bs[4] + shift_in_right<V>(bs[7], adjR ? r7 : z)) + shift_in_left<V>(bs[8], adjL ? l8 : z);
-            S.U[ub][c + 1] = upw;
-            S.M[ub][c + 1] = mid + bb;
-            S.D[ub][c + 1] = dwn;
+            S.A[1][eo] = mid + bb;
+            if (bD) S.A[0][ed] = upw;     // the group above me in the next row: what arrives from below it
+            if (bU) S.A[2][eu] = dwn;
           }
-          // spills into the columns of a body group that has no lane in this row
-          if (!adjR && c + 1 >= 0 && c + 1 < seff && !(((rw.bits[(c + 2) >> 5]) >> ((c + 2) & 31)) & 1u)) {
-            reinterpret_cast<R*>(&S.U[ub][c + 2])[0] = last_of<V>(bs[5]);
-            reinterpret_cast<R*>(&S.D[ub][c + 2])[0] = last_of<V>(bs[8]);
+          // a body group next to mine without a fluid node in this row has no lane: its columns in the rows
+          // above / below still receive the B* that leave my edge node diagonally
+          if (c + 1 < seff && !(((rw.bits[(c + 2) >> 5]) >> ((c + 2) & 31)) & 1u)) {
+            if (nbD & 2u) reinterpret_cast<R*>(&S.A[0][ed + (int)bD])[0] = last_of<V>(bs[5]);
+            if (nbU & 2u) reinterpret_cast<R*>(&S.A[2][eu + (int)bU])[0] = last_of<V>(bs[8]);
           }
-          if (!adjL && c - 1 >= 0 && c - 1 < seff && !(((rw.bits[c >> 5]) >> (c & 31)) & 1u)) {
-            reinterpret_cast<R*>(&S.U[ub][c])[NL - 1] = first_of<V>(bs[6]);
-            reinterpret_cast<R*>(&S.D[ub][c])[NL - 1] = first_of<V>(bs[7]);
+          if (c >= 1 && !(((rw.bits[c >> 5]) >> (c & 31)) & 1u)) {
+            if (nbD & 1u) reinterpret_cast<R*>(&S.A[0][ed - 1])[NL - 1] = first_of<V>(bs[6]);
+            if (nbU & 1u) reinterpret_cast<R*>(&S.A[2][eu - 1])[NL - 1] = first_of<V>(bs[7]);
           }
         }
         // done with every row before the first row of my next pass
         __syncwarp();
-        if (lane == 0) {
-          const int pn = p + SP_W;
-          const int dn_row = pn < NP ? row_of(30 * pn - 1) - 1 : TY + 2;
-          st_release(&S.done[warp], dn_row);
-        }
+        Rnext = p + SP_W < NP ? row_scan(R0, 30 * (p + SP_W) - 1) : TY + 3;
+        if (lane == 0) st_release(&S.done[warp], Rnext - 1);
       }
     }
     __syncthreads();
@@ -570,13 +583,13 @@ __global__ void __launch_bounds__(256) k_sp_meta(const uint8_t* __restrict__ cls
 }
 
 __global__ void __launch_bounds__(128) k_sp_desc(const uint2* __restrict__ ptab, const uint2* __restrict__ gmeta, int nx,
-                                                 int ny, int nw, int G, int nstrips, SpDesc* __restrict__ desc,
+                                                 int ny, int nw, int G, int nstrips, int sw, SpDesc* __restrict__ desc,
                                                  uint16_t* __restrict__ cnt) {
   const long long t = (long long)blockIdx.x * 128 + threadIdx.x;
   if (t >= (long long)nstrips * ny) return;
   const int strip = (int)(t / ny), r = (int)(t % ny);
   const int ng = nx / G;
-  const int c0 = strip * SP_S, seff = min(SP_S, ng - c0);
+  const int c0 = strip * sw, seff = min(sw, ng - c0);
   const uint2* prow = ptab + (size_t)r * nw;
   auto wrapg = [&](int g) -> int { g %= ng; return g < 0 ? g + ng : g; };
   auto act = [&](int g) -> unsigned { return (prow[g >> 5].x >> (g & 31)) & 1u; };
