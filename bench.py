@@ -221,7 +221,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
 
     fused = schedule != binding.SCHEDULE_BASELINE
     values = 20 if fused else 38
-    cls_bytes = 2 if schedule in (binding.SCHEDULE_AUTO, binding.SCHEDULE_PAIR, binding.SCHEDULE_WARP, binding.SCHEDULE_PACK, binding.SCHEDULE_SPARSE) else 1
+    cls_bytes = 2 if schedule in (binding.SCHEDULE_AUTO, binding.SCHEDULE_PAIR, binding.SCHEDULE_PACK, binding.SCHEDULE_SPARSE) else 1
     bytes_layout = n_fluid * values * rs + cls_bytes * n   # + the class word of every node (cl16: 2 B)
     bytes_canon = n_fluid * (36 * rs + 1)
     peak, peak_src = measured_peak()
@@ -231,7 +231,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist):
         e2e_mlups=n * args.steps / t_e2e / 1e6, launches=n_launch, clocks=clocks, create_s=t_create,
         split_ms_per_step={k: v / ks for k, v in split.items()},
         roofline={"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                  "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_FUSED: "k_fused_step", binding.SCHEDULE_WARP: "k_fused_warp"}.get(schedule, "k_fused_pair"),
+                  "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_FUSED: "k_fused_step", binding.SCHEDULE_SPARSE: "k_fused_sparse"}.get(schedule, "k_fused_pair"),
                   "bytes_per_launch": bytes_layout, "values_per_update": values,
                   "kernel_ms": t_collide * 1e3,
                   "layout_copy": None if t_copy is None else {
@@ -258,7 +258,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=8192)
     ap.add_argument("--precision", default="both", choices=["64", "32", "both"])
-    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "warp", "pair", "pack", "sparse"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "pair", "pack", "sparse"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--reference-budget", type=float, default=120.0, help="seconds of CPU work the --impl reference arm may spend")
     ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r1_traffic.csv"),
@@ -287,7 +287,7 @@ def main():
         dist = dist_mod
 
     sched = {"auto": binding.SCHEDULE_AUTO, "baseline": binding.SCHEDULE_BASELINE, "fused": binding.SCHEDULE_FUSED,
-             "warp": binding.SCHEDULE_WARP, "pair": binding.SCHEDULE_PAIR, "pack": binding.SCHEDULE_PACK, "sparse": binding.SCHEDULE_SPARSE}[args.schedule]
+             "pair": binding.SCHEDULE_PAIR, "pack": binding.SCHEDULE_PACK, "sparse": binding.SCHEDULE_SPARSE}[args.schedule]
     w = wl.config5(seed=replica_seed(rank), n=args.n)   # replicas: same recipe, rank-specific seed
     precs = [64, 32] if args.precision == "both" else [int(args.precision)]
     results = {p: bench_precision(args, w, p, sched, local, dist) for p in precs}

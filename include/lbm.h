@@ -21,10 +21,16 @@
  *   c = (0,0),(1,0),(0,1),(-1,0),(0,-1),(1,1),(-1,1),(-1,-1),(1,-1).
  * Population arrays are structure-of-arrays: pop[q*nx*ny + idx].
  *
+ * Deviations from the call list SURVEY.md 8(b) proposed (all recorded in DESIGN.md 1): lbm_plan (exact sizing
+ * from the mask, needs a device) exists beside lbm_workspace_bytes (host-only upper bound); lbm_params has
+ * three more fields (precision, ghost_rule, schedule); B_i are returned only after lbm_keep_B because they
+ * are not part of the stored state; test and measurement hooks live in include/lbm_test.h.
+ *
  * Memory and ownership: every pointer is the caller's.  Pointers marked HOST must be host
  * memory (pageable or pinned) and are only used during the call; they are never retained.
- * `d_workspace` (DEVICE) is the only device memory the context uses for its state; it must stay
- * allocated until lbm_destroy and be at least `workspace_bytes` (from lbm_plan) long, 256-byte
+ * `d_workspace` (DEVICE) is the only device memory a context uses — state, lists and the temporaries of
+ * lbm_create alike (lbm_plan and the hook lbm_node_update_batch, which have no workspace, allocate and
+ * free their own); it must stay allocated until lbm_destroy and be at least `workspace_bytes` (from lbm_plan) long, 256-byte
  * aligned.  `cuda_stream` is a borrowed cudaStream_t (0 = default stream); all work of a context
  * is enqueued on it.  A context is not thread-safe; different contexts are independent.
  *
@@ -53,11 +59,11 @@ enum {
   LBM_SCHEDULE_BASELINE = 1,  /* 3 launches/step: collide+stream, phi = sum B, ghost; N and B in HBM */
   LBM_SCHEDULE_FUSED = 2,     /* 2 launches/step: tiled collide+stream that also produces phi(t+1)
                                  from B* held in shared memory (B never touches HBM), ghost        */
-  LBM_SCHEDULE_WARP = 3,      /* 2 launches/step like FUSED but barrier-free: one warp marches down a
-                                 30-column strip, phi(t+1) is assembled in registers by warp
-                                 shuffles, loads run ahead through a per-warp cp.async ring        */
-  LBM_SCHEDULE_PAIR = 4,      /* like WARP, but every lane owns an aligned pair of nodes: each
-                                 population is fetched once, unshifted, as an 8/16-byte vector;
+                              /* 3 was the WARP schedule of round 1 (superseded by PAIR, removed): LBM_EINVAL */
+  LBM_SCHEDULE_PAIR = 4,      /* 2 launches/step, barrier-free: one warp marches down a strip of columns,
+                                 every lane owns an aligned group of nodes (2 in fp64, 4 in fp32); each
+                                 population is fetched once, unshifted, as an 8/16-byte vector through a
+                                 per-warp cp.async ring; phi(t+1) is assembled in registers;
                                  propagation in x is a warp shuffle; fp32 arithmetic is packed
                                  (FFMA2).  Needs even nx, else FUSED is used                        */
   LBM_SCHEDULE_PACK = 5,      /* the PAIR kernel on pair-compacted population planes: a plane stores
@@ -97,6 +103,11 @@ typedef struct {
  * outside [0,180], mobility outside (0, 0.3), precision not 32/64, wall rows not solid). */
 int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_t* workspace_bytes);
 
+/* Upper bound of the workspace size without touching a device or the mask (pure host arithmetic): what
+ * lbm_create needs for a mask with at most `n_ghost_bound` ghost nodes in which every node group may hold
+ * a fluid node.  lbm_plan's exact figure is never larger.  0 on bad parameters. */
+size_t lbm_workspace_bytes(const lbm_params* prm, int64_t n_ghost_bound);
+
 /* Builds a context in the caller's device workspace.  mask: HOST nx*ny bytes (copied).
  * disks: HOST array of n_disks analytic disks whose rasterisation produced the solid nodes of the
  * mask (closed disks, minimum-image distance^2 <= r^2); every ghost node that is not on a wall
@@ -130,12 +141,19 @@ int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, doub
 
 /* Post-stream populations N_i(x, t), B_i(x, t) of the current time, HOST 9*nx*ny doubles each
  * (SoA), either may be NULL; zeros on solid nodes.  Under every schedule but BASELINE (FUSED,
- * WARP, PAIR, hence AUTO) the B_i are not part of the stored state: they are available right after
+ * PAIR, PACK, SPARSE, hence AUTO) the B_i are not part of the stored state: they are available right after
  * lbm_init, and after lbm_step only if lbm_keep_B(ctx, 1) was set before that step (else
  * LBM_EINVAL for B != NULL).  Synchronises. */
 int lbm_get_populations(lbm_ctx* ctx, double* N, double* B);
 
-/* FUSED / WARP / PAIR schedules: when on != 0 the last time step of every lbm_step call also
+/* Overwrites the post-stream populations of the current time (the arrays lbm_get_populations returns):
+ * N and/or B, HOST 9*nx*ny doubles each (SoA), either may be NULL; values on solid nodes are ignored.
+ * With B given, phi = sum_i B_i (A13, :311) on fluid nodes and the ghost values are updated from it
+ * (Eq. 9, Jacobi: solid corners keep their previous values, R13) — exactly what the next time step of
+ * the oracle does after its set_populations.  Synchronises. */
+int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B);
+
+/* Every schedule but BASELINE: when on != 0 the last time step of every lbm_step call also
  * writes the post-collision B_i* to HBM (workspace is sized for it) so that lbm_get_populations can return
  * B_i.  No effect on the arithmetic.  Ignored by the BASELINE schedule (B always stored). */
 int lbm_keep_B(lbm_ctx* ctx, int32_t on);
@@ -158,32 +176,6 @@ int lbm_get_classification(lbm_ctx* ctx, uint8_t* cls, int32_t* n_ghost, int32_t
  * deterministic): out[0] = sum phi, [1] = sum (1 - phi), [2] = 1/2 sum rho |u|^2, [3] = max |u|,
  * [4] = min phi, [5] = max phi, [6] = number of fluid nodes, [7] = 1 if any NaN.  out: HOST. */
 int lbm_diag(lbm_ctx* ctx, double out[8]);
-
-/* Test hook: the local update of `count` independent nodes on the device, in the context-free
- * precision `precision` (32/64).  N: HOST 9*count doubles (node-major: N[9*k + q]), phi_nb: HOST
- * 9*count doubles, phi_nb[9*k + q] = phi(x + c_q); outputs Nstar, Bstar (9*count) and fields
- * (8*count: rho, tau, ux, uy, p, Fx, Fy, |grad phi|), any may be NULL. */
-int lbm_node_update_batch(const lbm_params* prm, int64_t count, const double* N,
-                          const double* phi_nb, double* Nstar, double* Bstar, double* fields);
-
-/* Measurement helper: advances n steps like lbm_step but brackets every kernel launch with CUDA
- * events on the context's stream and returns, after synchronising, the summed device time in
- * milliseconds per kernel kind: ms[0] = collide(+stream), ms[1] = phi-sum (BASELINE only),
- * ms[2] = ghost update.  The event records add a little launch overhead; use lbm_step for
- * throughput and this call for the per-kernel split. */
-int lbm_step_timed(lbm_ctx* ctx, int64_t n, double ms[3]);
-
-/* Measurement helper: the ceiling of the state layout.  Runs `iters` passes of a plain copy kernel
- * over the context's own arrays (every 32-byte sector of the 9 population planes and of phi that holds
- * a fluid node is read and written once; no halos, no arithmetic; destination is scratch memory, the
- * state is not disturbed) and returns the mean device time of one pass in milliseconds.  bench.py
- * reports it beside the roofline fraction: it is what a pure streaming pass over this layout costs.
- * LBM_EINVAL if nx*ny is not a whole number of sectors. */
-int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass);
-
-/* Device-timing helper: per-kernel-kind accumulated launch counts since the last reset;
- * counts[0] = collide(+stream), [1] = phi-sum, [2] = ghost, [3] = other. */
-int lbm_launch_counts(lbm_ctx* ctx, int64_t counts[4], int32_t reset);
 
 const char* lbm_last_error(const lbm_ctx* ctx); /* ctx may be NULL: last error of lbm_plan/create */
 const char* lbm_version(void);

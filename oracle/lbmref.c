@@ -137,10 +137,13 @@ void lbmref_chi(double alpha, double chi[9]) {
  * rules, is used for |eps| < 1e-8. */
 double lbmref_ghost_rule(double phiF, double eps, int32_t rule) {
   if (rule == 0) return phiF / (phiF + (1.0 - phiF) * exp(eps));
-  if (fabs(eps) < 1e-8) return phiF - eps * phiF * (1.0 - phiF);
   {
+    /* Eq. 10: phi_G = (2/eps) (a - sqrt(a^2 - 2 eps phi_F)) - phi_F, a = 1 + eps/2.  As
+     * printed it is 0/0 at theta = 90 deg (eps = 0, "special care", :87) and loses digits near it; with
+     * a - s = (a^2 - s^2)/(a + s) = 2 eps phi_F/(a + s) the same expression has no cancellation and
+     * no singular point. */
     double a = 1.0 + 0.5 * eps;
-    return (2.0 / eps) * (a - sqrt(a * a - 2.0 * eps * phiF)) - phiF;
+    return 4.0 * phiF / (a + sqrt(a * a - 2.0 * eps * phiF)) - phiF;
   }
 }
 

@@ -19,17 +19,18 @@ _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 _SO = os.path.join(_HERE, "liblbm_b200.so")
 
-SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_WARP, SCHEDULE_PAIR, SCHEDULE_PACK, SCHEDULE_SPARSE = 0, 1, 2, 3, 4, 5, 6
+SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_PAIR, SCHEDULE_PACK, SCHEDULE_SPARSE = 0, 1, 2, 4, 5, 6
 FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
-EXPORTS = ("lbm_plan", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
-           "lbm_get_populations", "lbm_keep_B", "lbm_sample_populations", "lbm_get_classification",
-           "lbm_diag", "lbm_node_update_batch", "lbm_step_timed", "lbm_layout_copy_timed", "lbm_launch_counts", "lbm_last_error", "lbm_version",
-           "lbm_destroy")
+# include/lbm.h (the product boundary) and include/lbm_test.h (test and measurement hooks)
+EXPORTS = ("lbm_plan", "lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
+           "lbm_get_populations", "lbm_set_populations", "lbm_keep_B", "lbm_sample_populations",
+           "lbm_get_classification", "lbm_diag", "lbm_last_error", "lbm_version", "lbm_destroy")
+TEST_EXPORTS = ("lbm_node_update_batch", "lbm_step_timed", "lbm_layout_copy_timed", "lbm_launch_counts")
 
 
 def _sources():
-    out = [os.path.join(_INC, "lbm.h")]
+    out = [os.path.join(_INC, "lbm.h"), os.path.join(_INC, "lbm_test.h")]
     for f in sorted(os.listdir(_CSRC)):
         if f.endswith((".cu", ".cuh", ".h")):
             out.append(os.path.join(_CSRC, f))
@@ -101,6 +102,9 @@ def load_library() -> C.CDLL:
         L = C.CDLL(_SO)
         vp, i64 = C.c_void_p, C.c_int64
         L.lbm_plan.argtypes = [C.POINTER(_Params), vp, C.POINTER(i64), C.POINTER(C.c_size_t)]
+        L.lbm_workspace_bytes.argtypes = [C.POINTER(_Params), i64]
+        L.lbm_workspace_bytes.restype = C.c_size_t
+        L.lbm_set_populations.argtypes = [vp, vp, vp]
         L.lbm_create.argtypes = [C.POINTER(vp), C.POINTER(_Params), vp, vp, C.c_int32, vp,
                                  C.c_size_t, vp]
         L.lbm_init.argtypes = [vp, vp, vp]
@@ -140,6 +144,12 @@ def _f64(a, size=None):
     if size is not None and a.size != size:
         raise ValueError(f"expected {size} values, got {a.size}")
     return a
+
+
+def workspace_bytes(prm: LBMParams, n_ghost_bound: int) -> int:
+    """Host-only upper bound of the workspace size (no device, no mask)."""
+    ps = prm.c_struct()
+    return int(load_library().lbm_workspace_bytes(C.byref(ps), int(n_ghost_bound)))
 
 
 def node_update_batch(prm: LBMParams, N, phi_nb):
@@ -246,6 +256,13 @@ class LBM:
         B = np.empty((9, self.ny, self.nx)) if want_B else None
         _check(load_library().lbm_get_populations(self._h, N.ctypes.data, B.ctypes.data if want_B else None), self._h)
         return N, B
+
+    def set_populations(self, N=None, B=None):
+        """Overwrites the post-stream populations of the current time (arrays shaped like get_populations')."""
+        Na = _f64(N, 9 * self.n) if N is not None else None
+        Ba = _f64(B, 9 * self.n) if B is not None else None
+        _check(load_library().lbm_set_populations(self._h, Na.ctypes.data if Na is not None else None,
+                                                  Ba.ctypes.data if Ba is not None else None), self._h)
 
     def sample_populations(self, idx, want_B: bool = False):
         idx = np.ascontiguousarray(idx, dtype=np.int64).reshape(-1)

@@ -12,11 +12,11 @@
 #include <vector>
 
 #include "../../include/lbm.h"
+#include "../../include/lbm_test.h"
 #include "lbm_fused.cuh"
 #include "lbm_kernels.cuh"
 #include "lbm_pair.cuh"
 #include "lbm_sparse.cuh"
-#include "lbm_warp.cuh"
 
 using namespace lbm;
 
@@ -133,7 +133,7 @@ int validate(const lbm_params* P, const char** why) {
   if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
   if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
   if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
-  if (P->schedule < 0 || P->schedule > 6) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 6 || P->schedule == 3) { *why = "unknown schedule"; return LBM_EINVAL; }
   if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
   return LBM_OK;
 }
@@ -377,12 +377,12 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
     } else if (c->packed) {   // PACK: compact planes step compact -> compact; the dense mirror N[cur] goes stale
       done = launch_fused_pack(C, c->cl16, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po, c->st, c->ptab,
                                c->nw, (unsigned)(c->cps * pack_group((int)sizeof(R), c->P.nx) * sizeof(R)));
+      if (!done) return LBM_ECUDA;   // never step the stale dense mirror instead
       c->ccur ^= 1;
       c->dense_valid = 0;
       c->cur ^= 1;     // undone below: the dense buffer index does not move
     }
     if (!done && c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
-    if (!done && c->sched == LBM_SCHEDULE_WARP) done = launch_fused_warp<R>(C, c->cl16, Ns, Nd, Bd, pi, po, c->st) == 0;
     if (!done) launch_fused_step<R>(C, c->cls, c->links, Ns, Nd, Bd, pi, po, c->st);
     c->cur ^= 1;
     c->pcur ^= 1;
@@ -411,7 +411,7 @@ template <typename V, typename R>
 bool launch_sparse_v(lbm_ctx* c, const Consts<R>& C, const R* Ns, R* Nd, R* Bd, const R* pi, R* po) {
   const size_t smem = sizeof(SpSmem<V>);
   auto kern = Bd ? k_fused_sparse<V, true> : k_fused_sparse<V, false>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+  if (!ensure_smem_attr(reinterpret_cast<const void*>(kern), smem)) return false;
   const unsigned cpsB = (unsigned)(c->cps * 16);
   kern<<<c->sp_ncta, SP_THREADS, smem, c->st>>>(C, Ns, Nd, Bd, pi, po, c->sp_desc, c->sp_cnt, c->sp_meta, c->sp_march,
                                                c->sp_first, cpsB, c->sp_sw);
@@ -512,6 +512,13 @@ int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_
   return LBM_OK;
 }
 
+size_t lbm_workspace_bytes(const lbm_params* prm, int64_t n_ghost_bound) {
+  const char* why;
+  if (validate(prm, &why) != LBM_OK || n_ghost_bound < 0) return 0;
+  const long long groups = ((long long)prm->nx * prm->ny + 1) / 2;   // no more groups than node pairs
+  return layout(nullptr, nullptr, prm, (long long)n_ghost_bound, use_pack(prm) ? groups : 0);
+}
+
 int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const lbm_disk* disks,
                int32_t n_disks, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   lbm_ctx* ctx = nullptr;
@@ -553,6 +560,14 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     if (e_ != cudaSuccess) { int rc_ = cuda_fail(nullptr, e_, #call); delete c; return rc_; } \
   } while (0)
 
+  // temporaries of this call are carved from the dense population planes, which hold nothing before lbm_init
+  Arena scratch{(char*)c->N[0], 0};
+  const size_t scratch_cap = 9 * plane_stride(prm) * (size_t)(c->is32 ? 4 : 8);
+  auto scratch_take = [&](size_t bytes) -> void* {
+    char* p0 = scratch.take<char>(bytes);
+    return scratch.off <= scratch_cap ? p0 : nullptr;
+  };
+
   // (1) classification; the mask is staged in the (not yet used) stage area
   uint8_t* d_mask = reinterpret_cast<uint8_t*>(c->stage);
   const unsigned nblk = (unsigned)((n + 255) / 256);
@@ -591,16 +606,16 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     int ncx = 1;
     std::vector<int> h_start, h_list;
     build_disk_cells(prm, disks, n_disks, &ncx, h_start, h_list);
-    int* d_cells = nullptr;   // [start | list], freed after the geometry kernel
-    CKC(cudaMalloc(&d_cells, (h_start.size() + h_list.size()) * sizeof(int)));
+    int* d_cells = (int*)scratch_take((h_start.size() + h_list.size()) * sizeof(int));   // [start | list]
+    if (!d_cells) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the disk cell lists"); }
     int* d_start = d_cells;
     int* d_list = d_cells + h_start.size();
     cudaMemcpyAsync(d_start, h_start.data(), h_start.size() * sizeof(int), cudaMemcpyHostToDevice, c->st);
     cudaMemcpyAsync(d_list, h_list.data(), h_list.size() * sizeof(int), cudaMemcpyHostToDevice, c->st);
     int* d_smooth = nullptr;   // mask-only normals (n_disks == 0): the solid indicator smoothed twice
     if (n_disks == 0) {
-      cudaError_t e = cudaMalloc(&d_smooth, 2 * n * sizeof(int));
-      if (e != cudaSuccess) { cudaFree(d_cells); delete c; return cuda_fail(nullptr, e, "cudaMalloc(mask normals)"); }
+      d_smooth = (int*)scratch_take(2 * n * sizeof(int));
+      if (!d_smooth) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the mask-normal temporaries"); }
       k_mask_smooth<<<nblk, 256, 0, c->st>>>(c->cls, nullptr, d_smooth + n, prm->nx, prm->ny);
       k_mask_smooth<<<nblk, 256, 0, c->st>>>(nullptr, d_smooth + n, d_smooth, prm->nx, prm->ny);
     }
@@ -617,26 +632,26 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     cudaMemcpyAsync(&bad, c->scal + 1, sizeof(int), cudaMemcpyDeviceToHost, c->st);
     {
       const cudaError_t e = cudaStreamSynchronize(c->st);
-      cudaFree(d_cells);
-      cudaFree(d_smooth);
       if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "ghost geometry"); }
     }
     if (bad) {
       delete c;
       return fail(nullptr, LBM_EINVAL, "mask and geometry disagree: a ghost node lies in no disk");
     }
-    // tile-major processing order for the ghost update (one-time; temporaries are freed again)
+    // tile-major processing order for the ghost update (one-time)
     {
       unsigned *k_in = nullptr, *k_out = nullptr;
       int *v_in = nullptr, *v_out = nullptr;
       void* tmp = nullptr;
       size_t tmp_bytes = 0;
-      cudaError_t e = cudaMalloc(&k_in, 4 * sizeof(int) * (size_t)ng);
-      if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(ghost order)"); }
+      scratch.off = 0;   // the geometry temporaries are done with
+      k_in = (unsigned*)scratch_take(4 * sizeof(int) * (size_t)ng);
+      if (!k_in) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the ghost ordering"); }
+      cudaError_t e = cudaSuccess;
       k_out = k_in + ng; v_in = reinterpret_cast<int*>(k_out + ng); v_out = v_in + ng;
       k_ghost_tile_keys<<<(ng + 255) / 256, 256, 0, c->st>>>(ng, c->gidx, prm->nx, k_in, v_in);
       e = cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, k_in, k_out, v_in, v_out, ng, 0, 32, c->st);
-      if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 1);
+      if (e == cudaSuccess && !(tmp = scratch_take(tmp_bytes ? tmp_bytes : 1))) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the ghost ordering"); }
       if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k_in, k_out, v_in, v_out, ng, 0, 32, c->st);
       if (e == cudaSuccess) {
         if (c->is32)
@@ -648,24 +663,23 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
         e = cudaGetLastError();
       }
       if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-      cudaFree(tmp);
-      cudaFree(k_in);
       if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "ghost processing order"); }
     }
   }
   if (use_pack(prm)) {   // PACK schedule: pair mask words and their compact base indices
     const long long nwords = (long long)prm->ny * c->nw;
-    unsigned* pmask = nullptr;
     void* tmp = nullptr;
     size_t tmp_bytes = 0;
-    cudaError_t e = cudaMalloc(&pmask, 3 * sizeof(int) * (size_t)nwords + 16);
-    if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(pair table)"); }
+    scratch.off = 0;
+    unsigned* pmask = (unsigned*)scratch_take(3 * sizeof(int) * (size_t)nwords + 16);
+    if (!pmask) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the group table temporaries"); }
+    cudaError_t e = cudaSuccess;
     int* pcount = reinterpret_cast<int*>(pmask + nwords);
     int* pbase = pcount + nwords;
     const unsigned nb = (unsigned)((nwords + 255) / 256);
     k_pair_mask<<<nb, 256, 0, c->st>>>(c->cls, prm->nx, prm->ny, c->nw, pack_group(c->is32 ? 4 : 8, prm->nx), pmask, pcount);
     e = cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, pcount, pbase, (int)nwords, c->st);
-    if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 1);
+    if (e == cudaSuccess && !(tmp = scratch_take(tmp_bytes ? tmp_bytes : 1))) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the group table temporaries"); }
     if (e == cudaSuccess) e = cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, pcount, pbase, (int)nwords, c->st);
     if (e == cudaSuccess) {
       k_pair_tab<<<nb, 256, 0, c->st>>>(pmask, pbase, nwords, c->ptab);
@@ -675,8 +689,6 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     if (e == cudaSuccess) e = cudaMemcpyAsync(&last[0], pbase + (nwords - 1), sizeof(int), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&last[1], pcount + (nwords - 1), sizeof(int), cudaMemcpyDeviceToHost, c->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-    cudaFree(tmp);
-    cudaFree(pmask);
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "pair table"); }
     if ((long long)last[0] + last[1] != nfp) { delete c; return fail(nullptr, LBM_EINVAL, "internal: fluid group counts of host and device differ"); }
     c->packed = 1;
@@ -763,7 +775,11 @@ int lbm_step(lbm_ctx* ctx, int64_t nsteps) {
   if (!ctx || nsteps < 0) return fail(ctx, LBM_EINVAL, "bad argument");
   for (int64_t s = 0; s < nsteps; s++) {
     const bool wb = ctx->fused && ctx->keep_B && s == nsteps - 1;
-    if (ctx->is32) step_once<float>(ctx, wb); else step_once<double>(ctx, wb);
+    const int rc = ctx->is32 ? step_once<float>(ctx, wb) : step_once<double>(ctx, wb);
+    if (rc != LBM_OK) {
+      const cudaError_t e = cudaGetLastError();
+      return cuda_fail(ctx, e, "kernel launch of lbm_step (the state did not advance past the failed step)");
+    }
   }
   CK(cudaGetLastError());
   return LBM_OK;
@@ -775,11 +791,13 @@ int lbm_step_timed(lbm_ctx* ctx, int64_t nsteps, double ms[3]) {
   tm.ms[0] = tm.ms[1] = tm.ms[2] = 0.0;
   for (int k = 0; k < 4; k++) CK(cudaEventCreate(&tm.ev[k]));
   CK(cudaStreamSynchronize(ctx->st));
-  for (int64_t s = 0; s < nsteps; s++) {
+  int rc = LBM_OK;
+  for (int64_t s = 0; s < nsteps && rc == LBM_OK; s++) {
     const bool wb = ctx->fused && ctx->keep_B && s == nsteps - 1;
-    if (ctx->is32) step_once<float>(ctx, wb, &tm); else step_once<double>(ctx, wb, &tm);
+    rc = ctx->is32 ? step_once<float>(ctx, wb, &tm) : step_once<double>(ctx, wb, &tm);
   }
   for (int k = 0; k < 4; k++) cudaEventDestroy(tm.ev[k]);
+  if (rc != LBM_OK) return cuda_fail(ctx, cudaGetLastError(), "kernel launch of lbm_step_timed");
   CK(cudaGetLastError());
   for (int k = 0; k < 3; k++) ms[k] = tm.ms[k];
   return LBM_OK;
@@ -852,6 +870,61 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
       CK(cudaStreamSynchronize(ctx->st));
     }
   }
+  return LBM_OK;
+}
+
+int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B) {
+  if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  if (!N && !B) return LBM_OK;
+  ensure_dense(ctx);   // planes that are not given keep their values
+  const size_t n = ctx->n;
+  int bx;
+  const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  const double chi[9] = {ctx->Cd.chi0, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1,
+                         ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5};
+  void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];
+  double* acc = ctx->stage + 4 * n;   // planes 0..3 stage the input, plane 4 accumulates phi
+  for (int which = 0; which < 2; which++) {
+    const double* host = which ? B : N;
+    if (!host) continue;
+    void* pop = which ? Bp : ctx->N[ctx->cur];
+    for (int q0 = 0; q0 < 9; q0 += 4) {
+      const int q1 = q0 + 4 < 9 ? q0 + 4 : 9;
+      CK(cudaMemcpyAsync(ctx->stage, host + (size_t)q0 * n, (size_t)(q1 - q0) * n * sizeof(double), cudaMemcpyHostToDevice, ctx->st));
+      for (int q = q0; q < q1; q++) {
+        const double* src = ctx->stage + (size_t)(q - q0) * n;
+        const double sub = which ? 0.0 : chi[q];
+        if (ctx->is32) {
+          if (pop) k_scatter_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, src, q, sub, (float*)pop);
+          if (which) k_phi_accumulate<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, src, q == 0, acc, q == 8 ? (float*)ctx->phi[ctx->pcur] : nullptr);
+        } else {
+          if (pop) k_scatter_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, src, q, sub, (double*)pop);
+          if (which) k_phi_accumulate<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, src, q == 0, acc, q == 8 ? (double*)ctx->phi[ctx->pcur] : nullptr);
+        }
+        ctx->launches[3] += which ? 2 : 1;
+      }
+      CK(cudaGetLastError());
+      CK(cudaStreamSynchronize(ctx->st));   // the staging planes are reused by the next chunk
+    }
+  }
+  if (N && ctx->packed) {   // the compact planes follow the dense ones
+    const int G = pack_group(ctx->is32 ? 4 : 8, ctx->P.nx);
+    const long long np = (long long)ctx->P.ny * (ctx->P.nx / G);
+    const unsigned nb = (unsigned)((np + 255) / 256);
+    if (ctx->is32)
+      k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cf.ps, ctx->cps,
+                                                          (float*)ctx->N[ctx->cur], (float*)ctx->Nc[ctx->ccur]);
+    else
+      k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cd.ps, ctx->cps,
+                                                           (double*)ctx->N[ctx->cur], (double*)ctx->Nc[ctx->ccur]);
+    ctx->launches[3]++;
+  }
+  if (B) {
+    ctx->B_valid = Bp ? 1 : 0;
+    if (ctx->is32) launch_ghost<float>(ctx); else launch_ghost<double>(ctx);   // ghost values follow the new phi (Eq. 9)
+  }
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(ctx->st));
   return LBM_OK;
 }
 

@@ -517,6 +517,41 @@ __global__ void __launch_bounds__(256) k_gather_plane(const Consts<R> C, const u
   out[k] = (double)v + add;
 }
 
+// lbm_set_populations: the inverse of k_gather_plane.  in[k] = post-stream N_q(x_k, t) (or B_q); the state keeps
+// the value at the node the pull will take it from: slot (q, x - c_q), or the node's own slot opp(q) behind a
+// bounce-back link.  Every slot a fluid node will pull from has exactly one writer.
+template <typename R>
+__global__ void __launch_bounds__(256) k_scatter_plane(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                       const uint8_t* __restrict__ links,
+                                                       const double* __restrict__ in, int q, double sub,
+                                                       R* __restrict__ pop) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = C.ps;   // plane stride
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (c >= 2) return;
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const R v = (R)(in[k] - sub);
+  if (q == 0) pop[k] = v;
+  else if ((lk >> (q - 1)) & 1u) pop[opp(q) * n + k] = v;
+  else pop[q * n + b.src[q]] = v;
+}
+// phi = sum_q B_q on fluid nodes (A13, :311), accumulated plane by plane in the oracle's order q = 0 .. 8
+template <typename R>
+__global__ void __launch_bounds__(256) k_phi_accumulate(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                        const double* __restrict__ in, int first,
+                                                        double* __restrict__ acc, R* __restrict__ phi_final) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const int k = j * C.nx + i;
+  if (cls[k] >= 2) return;
+  const double s = (first ? 0.0 : acc[k]) + in[k];
+  acc[k] = s;
+  if (phi_final) phi_final[k] = (R)s;
+}
+
 // same at selected nodes: out[q*m + t]
 template <typename R>
 __global__ void __launch_bounds__(128) k_gather_samples(const Consts<R> C, const uint8_t* __restrict__ cls,

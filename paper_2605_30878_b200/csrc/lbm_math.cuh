@@ -189,14 +189,15 @@ __device__ __forceinline__ void node_update(const Consts<R>& C, const R (&n)[9],
 }
 
 // Ghost-node rule.  rule 0: Eq. 9 (:78), phi_G = phi_F / (phi_F + (1 - phi_F) e^eps).
-// rule 1: Eq. 10 (:84) with the theta -> 90 deg guard of :87 (first-order series for tiny eps).
+// rule 1: Eq. 10 (:84), phi_G = (2/eps)(a - s) - phi_F with a = 1 + eps/2, s = sqrt(a^2 - 2 eps phi_F), written as
+// 4 phi_F/(a + s) - phi_F: the same value without the cancellation that makes the printed form 0/0 at
+// theta = 90 deg (:87) and useless in fp32 near it.
 template <typename R>
 __device__ __forceinline__ R ghost_rule(const Consts<R>& C, R phiF) {
   if (C.ghost_rule == 0) return phiF / (phiF + (R(1.0) - phiF) * C.E);
   const R eps = C.eps;
-  if (fabs((double)eps) < 1e-8) return phiF - eps * phiF * (R(1.0) - phiF);
   const R a = R(1.0) + R(0.5) * eps;
-  return (R(2.0) / eps) * (a - (R)sqrt((double)(a * a - R(2.0) * eps * phiF))) - phiF;
+  return R(4.0) * phiF / (a + (R)sqrt((double)(a * a - R(2.0) * eps * phiF))) - phiF;
 }
 
 }  // namespace lbm

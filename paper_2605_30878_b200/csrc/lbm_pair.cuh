@@ -19,10 +19,32 @@
 //   * stores are aligned vectors at the node's own position; a 32-byte sector that holds any fluid
 //     node is written whole (zeros on its solid nodes): partial sectors made HBM read-modify-write.
 #pragma once
+#include <mutex>
+#include <utility>
+#include <vector>
+
 #include "lbm_kernels.cuh"
-#include "lbm_warp.cuh"   // cp_async_commit / cp_async_wait
 
 namespace lbm {
+
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Opt-in to more than 48 KB of dynamic shared memory.  The attribute belongs to (kernel, device), so it is
+// remembered per pair; safe to call from several host threads.
+inline bool ensure_smem_attr(const void* kern, size_t smem) {
+  static std::mutex mu;
+  static std::vector<std::pair<const void*, int>> done;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return false;
+  std::lock_guard<std::mutex> lk(mu);
+  for (const auto& d : done)
+    if (d.first == kern && d.second == dev) return true;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+  done.emplace_back(kern, dev);
+  return true;
+}
 
 // pipeline depth and CTA shape per precision (overridable at build time for tuning sweeps)
 #ifndef LBM_PAIR_DP32
@@ -496,14 +518,7 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
   const size_t smem = sizeof(PairRing<V, DP, PACKED>) * WARPS;
   auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true, PACKED> : k_fused_pair<V, DP, WARPS, MINB, false, PACKED>;
-  static bool attr_set[2] = {false, false};
-  if (!attr_set[Bdst ? 1 : 0]) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
-#ifdef LBM_PAIR_CARVEOUT
-    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, LBM_PAIR_CARVEOUT);   // tuning experiment
-#endif
-    attr_set[Bdst ? 1 : 0] = true;
-  }
+  if (!ensure_smem_attr(reinterpret_cast<const void*>(kern), smem)) return false;
   kern<<<grid, 32 * WARPS, smem, st>>>(C, cl16, Nsrc, Ndst, Bdst, phi_in, phi_out, TY, ptab, nw, cpsB);
   return true;
 }

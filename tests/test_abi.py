@@ -11,8 +11,8 @@ from paper_2605_30878_b200 import binding
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared():
-    txt = open(os.path.join(ROOT, "include", "lbm.h")).read()
+def _declared(header="lbm.h"):
+    txt = open(os.path.join(ROOT, "include", header)).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
     return sorted(set(re.findall(r"\b(lbm_[a-z_A-Z0-9]+)\s*\(", txt)))
 
@@ -25,6 +25,10 @@ def test_library_builds_and_exports_every_declared_symbol():
     for name in names:
         assert hasattr(lib, name), name
     assert set(names) == set(binding.EXPORTS)
+    hooks = _declared("lbm_test.h")
+    assert set(hooks) == set(binding.TEST_EXPORTS)      # the hooks are declared apart from the product boundary
+    for name in hooks:
+        assert hasattr(lib, name), name
     assert b"sm_100a" in lib.lbm_version()
 
 

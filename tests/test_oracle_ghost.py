@@ -66,6 +66,25 @@ def test_eq10_solves_midpoint_rule():
             assert (phiF - g) == pytest.approx(eps * pm * (1 - pm), abs=1e-14)
 
 
+def test_eq10_near_ninety_degrees():
+    """Eq. 10 "needs special care" at theta = 90 deg (eps = 0).  The oracle's form of Eq. 10 has
+    no singular point: it still solves the midpoint rule to rounding for tiny eps, reduces to phi_G = phi_F at
+    eps = 0 and agrees with the expression as printed, evaluated with 50 digits, across the range."""
+    from decimal import Decimal, getcontext
+    getcontext().prec = 50
+    for eps in (1e-2, 1e-4, 1e-6, 1e-9, 1e-13, -1e-6, -1e-11):
+        for phiF in (0.05, 0.37, 0.5, 0.93):
+            g = ref.ghost_rule(phiF, eps, 1)
+            pm = 0.5 * (phiF + g)
+            assert abs((phiF - g) - eps * pm * (1 - pm)) <= 1e-15       # a few ulp of phi_F
+            e, f = Decimal(eps), Decimal(phiF)
+            a = 1 + e / 2
+            printed = (2 / e) * (a - (a * a - 2 * e * f).sqrt()) - f        # Eq. 10 as printed
+            assert abs(Decimal(g) - printed) <= Decimal(1e-15)
+    for phiF in (0.0, 0.2, 1.0):
+        assert ref.ghost_rule(phiF, 0.0, 1) == phiF
+
+
 def test_eq11_series_difference():
     """Eq. 9 - Eq. 10 = eps^3/12 [1 - 3(1-phi_F)phi_F] phi_F (1-phi_F) + O(eps^4) (PAPER.md:91)."""
     for phiF in (0.2, 0.5, 0.7):
