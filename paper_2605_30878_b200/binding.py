@@ -169,7 +169,9 @@ class LBM:
     """One simulation on the current CUDA device.  Device memory comes from a torch tensor, the
     stream is torch's current stream (PyTorch is plumbing only)."""
 
-    def __init__(self, prm: LBMParams, mask, disks=None, device=None):
+    def __init__(self, prm: LBMParams, mask, disks=None, device=None, own_stream: bool = False):
+        """own_stream: enqueue on a new non-default torch stream instead of the current one (the legacy default
+        stream cannot be captured, so lbm_step replays CUDA graphs on small grids only off it)."""
         import torch
         if not torch.cuda.is_available():
             raise LBMError("no CUDA device: liblbm_b200 has no CPU fallback")
@@ -188,7 +190,7 @@ class LBM:
             _check(L.lbm_plan(C.byref(ps), m.ctypes.data, C.byref(ng), C.byref(ws)))
             self.workspace_bytes = ws.value
             self._ws = torch.empty(ws.value, dtype=torch.uint8, device=self.device)
-            self._stream = torch.cuda.current_stream(self.device)
+            self._stream = torch.cuda.Stream(self.device) if own_stream else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
             _check(L.lbm_create(C.byref(h), C.byref(ps), m.ctypes.data, disks.ctypes.data if len(disks) else None, len(disks),
                                 C.c_void_p(self._ws.data_ptr()), ws.value,

@@ -97,6 +97,11 @@ struct lbm_ctx {
   int cur, pcur;      // population buffer holding the last post-collision state; phi buffer of time t
   int64_t t;
   int64_t launches[4];
+  // small grids are launch-bound: lbm_step replays CUDA graphs of kGraphSteps steps, one graph per
+  // parity of the ping-pong buffers it starts from
+  int graph_warm;          // two plain steps have run on this context (kernel attributes are set)
+  cudaGraphExec_t gexec[8];
+  int64_t gdelta[8][4];   // launches a replay adds
   char err[512];
 };
 
@@ -339,9 +344,8 @@ void launch_ghost(lbm_ctx* c) {
 bool launch_fused_sparse(lbm_ctx* c, const Consts<double>& C, const double* Ns, double* Nd, double* Bd, const double* pi, double* po);
 bool launch_fused_sparse(lbm_ctx* c, const Consts<float>& C, const float* Ns, float* Nd, float* Bd, const float* pi, float* po);
 
-struct StepTimer {   // optional event brackets around each launch (lbm_step_timed)
-  cudaEvent_t ev[4];
-  double ms[3];
+struct StepTimer {   // optional event brackets around each launch (lbm_step_timed): 4 events per step, read in bulk
+  cudaEvent_t* ev;   // the caller provides 4 events for this step
 };
 
 template <typename R>
@@ -393,15 +397,7 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
   if (tm) cudaEventRecord(tm->ev[2], c->st);
   launch_ghost<R>(c);
   c->t++;
-  if (tm) {
-    cudaEventRecord(tm->ev[3], c->st);
-    cudaEventSynchronize(tm->ev[3]);
-    float a = 0, b = 0, g = 0;
-    cudaEventElapsedTime(&a, tm->ev[0], tm->ev[1]);
-    cudaEventElapsedTime(&b, tm->ev[1], tm->ev[2]);
-    cudaEventElapsedTime(&g, tm->ev[2], tm->ev[3]);
-    tm->ms[0] += a; tm->ms[1] += b; tm->ms[2] += g;
-  }
+  if (tm) cudaEventRecord(tm->ev[3], c->st);
   return LBM_OK;
 }
 
@@ -729,7 +725,12 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   return LBM_OK;
 }
 
-void lbm_destroy(lbm_ctx* ctx) { delete ctx; }
+void lbm_destroy(lbm_ctx* ctx) {
+  if (!ctx) return;
+  for (auto& g : ctx->gexec)
+    if (g) cudaGraphExecDestroy(g);
+  delete ctx;
+}
 
 int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
   if (!ctx || !phi0) return fail(ctx, LBM_EINVAL, "null argument");
@@ -771,9 +772,53 @@ int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
   return LBM_OK;
 }
 
+namespace {
+constexpr int kGraphSteps = 32;                    // even: the ping-pong indices return to where they started
+constexpr size_t kGraphMaxNodes = (size_t)1 << 22; // larger grids run milliseconds per kernel: nothing to gain
+}
+
 int lbm_step(lbm_ctx* ctx, int64_t nsteps) {
   if (!ctx || nsteps < 0) return fail(ctx, LBM_EINVAL, "bad argument");
-  for (int64_t s = 0; s < nsteps; s++) {
+  int64_t s = 0;
+  // the legacy default stream cannot be captured; with keep_B the last step differs from the others
+  if (ctx->st != nullptr && ctx->st != cudaStreamLegacy && !ctx->keep_B && ctx->n <= kGraphMaxNodes) {
+    if (!ctx->graph_warm && nsteps - s >= kGraphSteps + 2) {   // first launches outside any capture
+      for (int k = 0; k < 2; k++, s++)
+        if ((ctx->is32 ? step_once<float>(ctx, false) : step_once<double>(ctx, false)) != LBM_OK)
+          return cuda_fail(ctx, cudaGetLastError(), "kernel launch of lbm_step");
+      ctx->graph_warm = 1;
+    }
+    while (ctx->graph_warm && nsteps - s >= kGraphSteps) {
+      const int key = (ctx->cur & 1) | ((ctx->pcur & 1) << 1) | ((ctx->ccur & 1) << 2);
+      if (!ctx->gexec[key]) {   // capture kGraphSteps steps once, then run them
+        int64_t before[4];
+        for (int k = 0; k < 4; k++) before[k] = ctx->launches[k];
+        if (cudaStreamBeginCapture(ctx->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); break; }
+        int rc = LBM_OK;
+        for (int k = 0; k < kGraphSteps && rc == LBM_OK; k++)
+          rc = ctx->is32 ? step_once<float>(ctx, false) : step_once<double>(ctx, false);
+        cudaGraph_t g = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(ctx->st, &g);
+        if (rc != LBM_OK || e != cudaSuccess || !g) {
+          if (g) cudaGraphDestroy(g);
+          return cuda_fail(ctx, e != cudaSuccess ? e : cudaGetLastError(), "capture of the step graph");
+        }
+        const cudaError_t ei = cudaGraphInstantiate(&ctx->gexec[key], g, 0);
+        cudaGraphDestroy(g);
+        if (ei != cudaSuccess) { ctx->gexec[key] = nullptr; return cuda_fail(ctx, ei, "cudaGraphInstantiate"); }
+        for (int k = 0; k < 4; k++) ctx->gdelta[key][k] = ctx->launches[k] - before[k];
+        // the capture advanced the bookkeeping by kGraphSteps steps: this launch executes them
+      } else {
+        ctx->t += kGraphSteps;
+        for (int k = 0; k < 4; k++) ctx->launches[k] += ctx->gdelta[key][k];
+        ctx->B_valid = ctx->fused ? 0 : 1;
+        if (ctx->packed) ctx->dense_valid = 0;
+      }
+      CK(cudaGraphLaunch(ctx->gexec[key], ctx->st));
+      s += kGraphSteps;
+    }
+  }
+  for (; s < nsteps; s++) {
     const bool wb = ctx->fused && ctx->keep_B && s == nsteps - 1;
     const int rc = ctx->is32 ? step_once<float>(ctx, wb) : step_once<double>(ctx, wb);
     if (rc != LBM_OK) {
@@ -787,19 +832,33 @@ int lbm_step(lbm_ctx* ctx, int64_t nsteps) {
 
 int lbm_step_timed(lbm_ctx* ctx, int64_t nsteps, double ms[3]) {
   if (!ctx || nsteps < 0 || !ms) return fail(ctx, LBM_EINVAL, "bad argument");
-  StepTimer tm;
-  tm.ms[0] = tm.ms[1] = tm.ms[2] = 0.0;
-  for (int k = 0; k < 4; k++) CK(cudaEventCreate(&tm.ev[k]));
+  // events of a chunk of steps are recorded without any host synchronisation in between and read afterwards
+  const int chunk = 256;
+  std::vector<cudaEvent_t> ev(4 * chunk);
+  for (auto& e : ev) CK(cudaEventCreate(&e));
+  double acc[3] = {0.0, 0.0, 0.0};
   CK(cudaStreamSynchronize(ctx->st));
   int rc = LBM_OK;
-  for (int64_t s = 0; s < nsteps && rc == LBM_OK; s++) {
-    const bool wb = ctx->fused && ctx->keep_B && s == nsteps - 1;
-    rc = ctx->is32 ? step_once<float>(ctx, wb, &tm) : step_once<double>(ctx, wb, &tm);
+  for (int64_t s0 = 0; s0 < nsteps && rc == LBM_OK; s0 += chunk) {
+    const int m = (int)std::min<int64_t>(chunk, nsteps - s0);
+    for (int k = 0; k < m && rc == LBM_OK; k++) {
+      StepTimer tm{&ev[4 * k]};
+      const bool wb = ctx->fused && ctx->keep_B && s0 + k == nsteps - 1;
+      rc = ctx->is32 ? step_once<float>(ctx, wb, &tm) : step_once<double>(ctx, wb, &tm);
+    }
+    if (rc != LBM_OK) break;
+    if (cudaEventSynchronize(ev[4 * (m - 1) + 3]) != cudaSuccess) { rc = LBM_ECUDA; break; }
+    for (int k = 0; k < m; k++)
+      for (int j = 0; j < 3; j++) {
+        float t = 0.f;
+        cudaEventElapsedTime(&t, ev[4 * k + j], ev[4 * k + j + 1]);
+        acc[j] += t;
+      }
   }
-  for (int k = 0; k < 4; k++) cudaEventDestroy(tm.ev[k]);
+  for (auto& e : ev) cudaEventDestroy(e);
   if (rc != LBM_OK) return cuda_fail(ctx, cudaGetLastError(), "kernel launch of lbm_step_timed");
   CK(cudaGetLastError());
-  for (int k = 0; k < 3; k++) ms[k] = tm.ms[k];
+  for (int k = 0; k < 3; k++) ms[k] = acc[k];
   return LBM_OK;
 }
 

@@ -245,6 +245,25 @@ def test_config1_1000_steps_fp64(schedule):
     assert abs(g.diag()["sum_phi"] - m0) < 1e-10 * m0
 
 
+def test_config1_1000_steps_through_cuda_graphs():
+    """Small grids are launch-bound: off the legacy default stream lbm_step replays CUDA graphs
+    of 32 steps.  Same 1,000-step parity run as above, same bar, and the launch bookkeeping still counts every
+    kernel; odd step counts leave the ping-pong parity the graphs were captured for."""
+    from paper_2605_30878_b200 import binding
+    from oracle import ref
+    w = wl.config1(seed=0)
+    o = ref.RefLBM(ref.RefParams(**w.param_dict()), w.mask, w.disks)
+    g = binding.LBM(binding.LBMParams(precision=64, **w.param_dict()), w.mask, w.disks, own_stream=True)
+    g.init(w.phi0); o.init(w.phi0)
+    for k in (333, 1, 666):      # 333 = 2 + 10 graphs + 11 plain steps; then an odd start for the next graphs
+        g.step(k)
+    o.step(1000)
+    err, _ = field_errors(g, o)
+    assert max(err.values()) <= 1e-10, err
+    lc = g.launch_counts()
+    assert lc["collide"] == 1000 and lc["ghost"] == 1001
+
+
 @pytest.mark.parametrize("schedule", SCHEDULES)
 def test_config1_1000_steps_fp32(schedule):
     w = wl.config1(seed=0)
