@@ -239,7 +239,8 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
   Arena A{base, 0};
   const size_t ps = plane_stride(P);
   char* N0 = A.take<char>(9 * ps * rs);
-  char* N1 = A.take<char>(9 * ps * rs);
+  // compacted planes (PACK / SPARSE) carry the state: one dense mirror is enough (lbm_get, lbm_diag, ... refresh it)
+  char* N1 = use_pack(P) ? nullptr : A.take<char>(9 * ps * rs);
   char* B0 = A.take<char>(9 * ps * rs);
   char* B1 = fused ? nullptr : A.take<char>(9 * ps * rs);
   char* p0 = A.take<char>(n * rs);
@@ -1065,6 +1066,10 @@ int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass) {
   const size_t nsec = ctx->n / nps, psec = ctx->Cd.ps / nps;
   const float4* src = (const float4*)ctx->N[ctx->cur];
   float4* dst = (float4*)ctx->N[ctx->cur ^ 1];          // scratch: the next step overwrites it
+  if (!dst) {                                            // compacted state: no second dense buffer, the B planes serve
+    dst = (float4*)ctx->B[0];
+    ctx->B_valid = 0;
+  }
   const float4* psrc = (const float4*)ctx->phi[ctx->pcur];
   float4* pdst = (float4*)ctx->stage;                    // scratch (phi[pcur ^ 1] holds the previous ghost values)
   cudaEvent_t e0, e1;
