@@ -637,6 +637,26 @@ def test_paper_flat_plate_contact_angles(W, tol_deg):
         s.close()
 
 
+def test_paper_flat_plate_interface_width_sweep():
+    """§III.A, Fig. 7: the interface width swept over W = 4 ... 10 at the two extreme angles,
+    theta = 30 and 150 deg.  The paper's statement: the error of the measured angle stays below 2 degrees once
+    W >= 6; at W = 4, 5 it is a few degrees (Fig. 6-7)."""
+    worst = {}
+    for W in (4.0, 5.0, 6.0, 7.0, 8.0, 9.0, 10.0):
+        for theta in (30.0, 150.0):
+            w = wl.flat_plate(theta_deg=theta, W=W, scale=1.0)
+            s = _gpu_sim(w, 64)
+            m0 = s.diag()["sum_phi"]
+            s.step(30000)
+            d = s.diag()
+            th = ms.contact_angle_on_plate(s.get()["phi"], w.mask, w.W)[0]
+            worst[(W, theta)] = th - theta
+            assert d["nan"] == 0 and abs(d["sum_phi"] - m0) < 1e-10 * m0
+            assert abs(th - theta) < (2.0 if W >= 6.0 else 5.0), (W, theta, th)
+            s.close()
+    print("flat plate W sweep, theta_measured - theta:", worst)
+
+
 def test_paper_particle_at_interface_eq13():
     """§III.C: 4.8 R box, R = 25: displacement h* of the interface at the periodic boundary against Eq. 13;
     the paper's own error is ~9 % at 30 / 150 deg and ~6 % at 60 - 120 deg (:197)."""
