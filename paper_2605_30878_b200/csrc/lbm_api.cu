@@ -409,9 +409,8 @@ bool launch_sparse_v(lbm_ctx* c, const Consts<R>& C, const R* Ns, R* Nd, R* Bd, 
   const size_t smem = sizeof(SpSmem<V>);
   auto kern = Bd ? k_fused_sparse<V, true> : k_fused_sparse<V, false>;
   if (!ensure_smem_attr(reinterpret_cast<const void*>(kern), smem)) return false;
-  const unsigned cpsB = (unsigned)(c->cps * 16);
   kern<<<c->sp_ncta, SP_THREADS, smem, c->st>>>(C, Ns, Nd, Bd, pi, po, c->sp_desc, c->sp_cnt, c->sp_meta, c->sp_march,
-                                               c->sp_first, cpsB, c->sp_sw);
+                                               c->sp_first, c->sp_sw);
   return true;
 }
 bool launch_fused_sparse(lbm_ctx* c, const Consts<double>& C, const double* Ns, double* Nd, double* Bd, const double* pi,
@@ -463,10 +462,10 @@ void ensure_dense(lbm_ctx* c) {
   const unsigned nb = (unsigned)((np + 255) / 256);
   if (c->is32)
     k_pair_repack<float, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, G, c->Cf.ps, c->cps,
-                                                       (float*)c->N[c->cur], (float*)c->Nc[c->ccur]);
+                                                       (float*)c->N[c->cur], (float*)c->Nc[c->ccur], c->sparse);
   else
     k_pair_repack<double, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, G, c->Cd.ps, c->cps,
-                                                        (double*)c->N[c->cur], (double*)c->Nc[c->ccur]);
+                                                        (double*)c->N[c->cur], (double*)c->Nc[c->ccur], c->sparse);
   c->launches[3]++;
   c->dense_valid = 1;
 }
@@ -760,10 +759,10 @@ int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
     const unsigned nb = (unsigned)((np + 255) / 256);
     if (ctx->is32)
       k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cf.ps, ctx->cps,
-                                                          (float*)ctx->N[0], (float*)ctx->Nc[0]);
+                                                          (float*)ctx->N[0], (float*)ctx->Nc[0], ctx->sparse);
     else
       k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cd.ps, ctx->cps,
-                                                           (double*)ctx->N[0], (double*)ctx->Nc[0]);
+                                                           (double*)ctx->N[0], (double*)ctx->Nc[0], ctx->sparse);
     ctx->ccur = 0;
     ctx->dense_valid = 1;
   }
@@ -973,10 +972,10 @@ int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B) {
     const unsigned nb = (unsigned)((np + 255) / 256);
     if (ctx->is32)
       k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cf.ps, ctx->cps,
-                                                          (float*)ctx->N[ctx->cur], (float*)ctx->Nc[ctx->ccur]);
+                                                          (float*)ctx->N[ctx->cur], (float*)ctx->Nc[ctx->ccur], ctx->sparse);
     else
       k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cd.ps, ctx->cps,
-                                                           (double*)ctx->N[ctx->cur], (double*)ctx->Nc[ctx->ccur]);
+                                                           (double*)ctx->N[ctx->cur], (double*)ctx->Nc[ctx->ccur], ctx->sparse);
     ctx->launches[3]++;
   }
   if (B) {

@@ -724,12 +724,14 @@ __global__ void __launch_bounds__(256) k_pair_tab(const unsigned* __restrict__ p
   const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
   if (t < nwords) ptab[t] = make_uint2(pmask[t], (unsigned)pbase[t]);
 }
-// dense (pop[q * ps + k]) <-> compact (popc[(q * cps + ci) * G + c]) copies of the 9 planes; TO_COMPACT
-// packs, else unpacks (the solid nodes of a group travel with it; other dense entries are untouched)
+// dense (pop[q * ps + k]) <-> compact copies of the 9 planes; TO_COMPACT packs, else unpacks (the solid nodes of a
+// group travel with it; other dense entries are untouched).  Compact element (q, group ci, node c): plane-major
+// popc[(q * cps + ci) * G + c] (PACK), or group-major popc[(ci * 9 + q) * G + c] (SPARSE: the nine vectors of a
+// group are contiguous, so a row of a strip is one contiguous run).
 template <typename R, bool TO_COMPACT>
 __global__ void __launch_bounds__(256) k_pair_repack(const uint2* __restrict__ ptab, int nx, int ny, int nw, int G,
                                                      size_t ps, size_t cps, R* __restrict__ dense,
-                                                     R* __restrict__ compact) {
+                                                     R* __restrict__ compact, int group_major) {
   const long long t = (long long)blockIdx.x * 256 + threadIdx.x;   // one thread per group
   const int npr = nx / G;
   if (t >= (long long)ny * npr) return;
@@ -740,8 +742,9 @@ __global__ void __launch_bounds__(256) k_pair_repack(const uint2* __restrict__ p
   const size_t k = (size_t)r * nx + (size_t)G * p;
   for (int q = 0; q < 9; q++)
     for (int c = 0; c < G; c++) {
-      if (TO_COMPACT) compact[(q * cps + ci) * G + c] = dense[q * ps + k + c];
-      else dense[q * ps + k + c] = compact[(q * cps + ci) * G + c];
+      const size_t e = group_major ? (ci * 9 + q) * G + c : (q * cps + ci) * G + c;
+      if (TO_COMPACT) compact[e] = dense[q * ps + k + c];
+      else dense[q * ps + k + c] = compact[e];
     }
 }
 

@@ -75,7 +75,7 @@ struct SpRow {        // shared-memory copy of what the consumers need of a row
 
 template <typename V>
 struct SpSmem {
-  V N[9][SP_CAP];
+  V N[SP_CAP][9];       // group-major, like the compact planes in HBM: a row is one contiguous run
   uint2 meta[SP_CAP];
   V phi[SP_NR][SP_S + 4];
   V A[3][SP_CAP];       // per entry: what the rows above / at / below contribute to its phi(t+1)
@@ -85,7 +85,8 @@ struct SpSmem {
   int rstart[SP_NR];
   int done[32];
   int ret_row[SP_K];    // class k: rows R = k (mod K) below ret_row[k] are retired
-  int pad[4 - SP_K % 4];
+  int next_pass;        // pass counter of the march
+  int pad[3 - SP_K % 4];
 };
 
 // ---- mbarrier / bulk-copy / ordered shared-memory access ----
@@ -184,7 +185,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
                    typename LaneOf<V>::R* __restrict__ Ndst, typename LaneOf<V>::R* __restrict__ Bdst,
                    const typename LaneOf<V>::R* __restrict__ phi_in, typename LaneOf<V>::R* __restrict__ phi_out,
                    const SpDesc* __restrict__ desc, const uint16_t* __restrict__ cnt, const uint2* __restrict__ gmeta,
-                   const SpMarch* __restrict__ marches, const int* __restrict__ cta_first, unsigned cpsB, int sw) {
+                   const SpMarch* __restrict__ marches, const int* __restrict__ cta_first, int sw) {
   using L = LaneOf<V>;
   using R = typename L::R;
   constexpr int NL = L::NL;
@@ -237,6 +238,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
     if (tid == 32) {
       for (int k = 0; k < SP_NR; k++) mbar_init((unsigned)__cvta_generic_to_shared(&S.full[k]), 1);
       for (int k = 0; k < SP_K; k++) S.ret_row[k] = k;
+      S.next_pass = 0;
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < 32) S.done[tid] = 0;
@@ -312,24 +314,11 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
           const unsigned bytes = 9u * 16u * ((unsigned)runLen + (wl ? 1u : 0u) + (wr ? 1u : 0u)) + metaBytes + phiBytes;
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           mbar_arrive_tx(mb, bytes);
-          const char* src = reinterpret_cast<const char*>(Nsrc);
-          const unsigned dN = (unsigned)__cvta_generic_to_shared(&S.N[0][0]);
-          if (runLen > 0) {
-#pragma unroll
-            for (int q = 0; q < 9; q++)
-              bulk_g2s(dN + (unsigned)(q * SP_CAP + runRing) * 16u, src + (size_t)cpsB * (unsigned)q + (size_t)runCi * 16u,
-                       (unsigned)runLen * 16u, mb);
-          }
-          if (wl) {
-#pragma unroll
-            for (int q = 0; q < 9; q++)
-              bulk_g2s(dN + (unsigned)(q * SP_CAP + off0) * 16u, src + (size_t)cpsB * (unsigned)q + (size_t)d.ciL * 16u, 16u, mb);
-          }
-          if (wr) {
-#pragma unroll
-            for (int q = 0; q < 9; q++)
-              bulk_g2s(dN + (unsigned)(q * SP_CAP + off0 + n - 1) * 16u, src + (size_t)cpsB * (unsigned)q + (size_t)d.ciR * 16u, 16u, mb);
-          }
+          const char* src = reinterpret_cast<const char*>(Nsrc);   // group ci: 9 vectors of 16 bytes at ci * 144
+          if (runLen > 0)
+            bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[runRing][0]), src + (size_t)runCi * 144u, (unsigned)runLen * 144u, mb);
+          if (wl) bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[off0][0]), src + (size_t)d.ciL * 144u, 144u, mb);
+          if (wr) bulk_g2s((unsigned)__cvta_generic_to_shared(&S.N[off0 + n - 1][0]), src + (size_t)d.ciR * 144u, 144u, mb);
           if (metaBytes)
             bulk_g2s((unsigned)__cvta_generic_to_shared(&S.meta[off0 + (int)d.hl - (int)(d.ci0 & 1u)]), gmeta + mStart, metaBytes, mb);
           // phi: logical groups c0-2 .. c0+seff+1 of the periodic row, cut where they wrap
@@ -393,12 +382,18 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
         while ((int)S.T[r] <= s) r++;
         return r;
       };
-      // a warp has no claim on the rows before its first pass
-      int Rnext = warp < NP ? row_scan(1, max(30 * warp - 1, 0)) : TY + 3;
-      if (lane == 0) st_release(&S.done[warp], Rnext - 1);
-      for (int p = warp; p < NP; p += SP_W) {
+      // passes are handed out in order to whichever warp is free: the passes in flight stay consecutive, so the
+      // rows they span (which the ring must hold) stay few even when warps fall behind one another
+      int Rprev = 1;
+      for (;;) {
+        int p = 0;
+        if (lane == 0) p = atomicAdd(&S.next_pass, 1);
+        p = __shfl_sync(FULL, p, 0);
+        if (p >= NP) break;
         const int s0 = 30 * p - 1;
-        const int R0 = Rnext;
+        const int R0 = row_scan(Rprev, max(s0, 0));
+        Rprev = R0;
+        if (lane == 0) st_release(&S.done[warp], R0 - 1);   // no claim on the rows before this pass any more
         const int s = s0 + lane;
         int Rl = R0;
 #pragma unroll
@@ -456,18 +451,18 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
             nbD |= ((rd.bits[(c + 2) >> 5] >> ((c + 2) & 31)) & 1u) << 1;
           }
           // own-position populations of the node's row, and the neighbours' (propagation A16-A17)
-          const V o0 = S.N[0][eo], o1 = S.N[1][eo], o2 = S.N[2][eo], o3 = S.N[3][eo], o4 = S.N[4][eo],
-                  o5 = S.N[5][eo], o6 = S.N[6][eo], o7 = S.N[7][eo], o8 = S.N[8][eo];
+          const V o0 = S.N[eo][0], o1 = S.N[eo][1], o2 = S.N[eo][2], o3 = S.N[eo][3], o4 = S.N[eo][4],
+                  o5 = S.N[eo][5], o6 = S.N[eo][6], o7 = S.N[eo][7], o8 = S.N[eo][8];
           V nn[9];
           nn[0] = o0;
-          nn[1] = shift_in_left<V>(o1, reinterpret_cast<const R*>(&S.N[1][eo - 1])[NL - 1]);
-          nn[3] = shift_in_right<V>(o3, reinterpret_cast<const R*>(&S.N[3][eo + 1])[0]);
-          nn[2] = S.N[2][eu];
-          nn[5] = shift_in_left<V>(S.N[5][eu], reinterpret_cast<const R*>(&S.N[5][eu - 1])[NL - 1]);
-          nn[6] = shift_in_right<V>(S.N[6][eu], reinterpret_cast<const R*>(&S.N[6][eu + (int)bU])[0]);
-          nn[4] = S.N[4][ed];
-          nn[7] = shift_in_right<V>(S.N[7][ed], reinterpret_cast<const R*>(&S.N[7][ed + (int)bD])[0]);
-          nn[8] = shift_in_left<V>(S.N[8][ed], reinterpret_cast<const R*>(&S.N[8][ed - 1])[NL - 1]);
+          nn[1] = shift_in_left<V>(o1, reinterpret_cast<const R*>(&S.N[eo - 1][1])[NL - 1]);
+          nn[3] = shift_in_right<V>(o3, reinterpret_cast<const R*>(&S.N[eo + 1][3])[0]);
+          nn[2] = S.N[eu][2];
+          nn[5] = shift_in_left<V>(S.N[eu][5], reinterpret_cast<const R*>(&S.N[eu - 1][5])[NL - 1]);
+          nn[6] = shift_in_right<V>(S.N[eu][6], reinterpret_cast<const R*>(&S.N[eu + (int)bU][6])[0]);
+          nn[4] = S.N[ed][4];
+          nn[7] = shift_in_right<V>(S.N[ed][7], reinterpret_cast<const R*>(&S.N[ed + (int)bD][7])[0]);
+          nn[8] = shift_in_left<V>(S.N[ed][8], reinterpret_cast<const R*>(&S.N[ed - 1][8])[NL - 1]);
           if (lk_any) {   // half-way bounce-back (R12): the node's own opposite population
             const V own[9] = {o0, o1, o2, o3, o4, o5, o6, o7, o8};
 #pragma unroll
@@ -493,9 +488,9 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
           collide_lane<V>(C, nn, ph, fl, all_fl, ns, bs);
           if (outl && body && Rl >= 2 && Rl <= TY + 1) {
             const unsigned ci = rw.ci0 + (unsigned)(e - (int)(rw.hlr & 1u));
-            char* dst = reinterpret_cast<char*>(Ndst) + (size_t)ci * 16u;
+            char* dst = reinterpret_cast<char*>(Ndst) + (size_t)ci * 144u;
 #pragma unroll
-            for (int q = 0; q < 9; q++) store_vec<V>(dst + (size_t)cpsB * (unsigned)q, ns[q]);
+            for (int q = 0; q < 9; q++) store_vec<V>(dst + 16 * q, ns[q]);
             if (WRITE_B) {
               char* dstB = reinterpret_cast<char*>(Bdst + ((size_t)rw.jrow * (size_t)nx + (size_t)(c0 + c) * NL));
 #pragma unroll
@@ -550,9 +545,9 @@ __global__ void __launch_bounds__(SP_THREADS, 1)
         }
         // done with every row before the first row of my next pass
         __syncwarp();
-        Rnext = p + SP_W < NP ? row_scan(R0, 30 * (p + SP_W) - 1) : TY + 3;
-        if (lane == 0) st_release(&S.done[warp], Rnext - 1);
       }
+      __syncwarp();
+      if (lane == 0) st_release(&S.done[warp], TY + 2);
     }
     __syncthreads();
     if (tid == 32)
