@@ -64,10 +64,8 @@ struct lbm_ctx {
   double *gnx, *gny, *gdepth;
   uint8_t* csolid;
   // the same list in the ghost kernel's processing order (tile-major)
-  int* gidx_p;
-  int* corner_p;
-  void* wgt_p;
-  uint8_t* csolid_p;
+  uint2* gent_p;      // {node index, corner code}
+  void* gfr_p;        // (f_x, f_y) in the device precision
   // PACK schedule: pair-compacted population planes (dense N[cur] is a mirror, refreshed on demand)
   int packed;
   int dense_valid;
@@ -263,10 +261,8 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
   double* gny = A.take<double>(g);
   double* gdepth = A.take<double>(g);
   uint8_t* csolid = A.take<uint8_t>(g);
-  int* gidx_p = A.take<int>(g);
-  int* corner_p = A.take<int>(4 * g);
-  char* wgt_p = A.take<char>(4 * g * rs);
-  uint8_t* csolid_p = A.take<uint8_t>(g);
+  uint2* gent_p = A.take<uint2>(g);
+  char* gfr_p = A.take<char>(2 * g * rs);
   // PACK schedule (last, so that nothing above depends on the pair count)
   uint2* ptab = nullptr;
   char *Nc0 = nullptr, *Nc1 = nullptr;
@@ -293,7 +289,7 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
     c->N[0] = N0; c->N[1] = N1; c->B[0] = B0; c->B[1] = B1; c->phi[0] = p0; c->phi[1] = p1;
     c->cls = cls; c->links = links; c->cl16 = cl16; c->gidx = gidx; c->corner = corner; c->wgt = wgt; c->wgt_d = wgt_d;
     c->gnx = gnx; c->gny = gny; c->gdepth = gdepth; c->csolid = csolid;
-    c->gidx_p = gidx_p; c->corner_p = corner_p; c->wgt_p = wgt_p; c->csolid_p = csolid_p;
+    c->gent_p = gent_p; c->gfr_p = gfr_p;
     c->ptab = ptab; c->Nc[0] = Nc0; c->Nc[1] = Nc1; c->nw = nw; c->cps = cps; c->blk_cnt = blk_cnt;
     c->blk_off = blk_off; c->scal = scal; c->stage = stage; c->diag_out = diag_out;
     c->samp_idx = samp; c->samp_cap = samp_cap;
@@ -337,7 +333,7 @@ template <typename R>
 void launch_ghost(lbm_ctx* c) {
   if (c->ng == 0) return;
   k_ghost_update<R><<<(c->ng + 127) / 128, 128, 0, c->st>>>(
-      consts_of<R>(c), c->ng, c->gidx_p, (const int4*)c->corner_p, (const R*)c->wgt_p, c->csolid_p,
+      consts_of<R>(c), c->ng, c->gent_p, (const typename GhostFrac<R>::T*)c->gfr_p,
       (const R*)c->phi[c->pcur ^ 1], (R*)c->phi[c->pcur]);
   c->launches[2]++;
 }
@@ -615,14 +611,16 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
       k_mask_smooth<<<nblk, 256, 0, c->st>>>(c->cls, nullptr, d_smooth + n, prm->nx, prm->ny);
       k_mask_smooth<<<nblk, 256, 0, c->st>>>(nullptr, d_smooth + n, d_smooth, prm->nx, prm->ny);
     }
+    double2* d_gfrac = (double2*)scratch_take((size_t)ng * sizeof(double2));   // (f_x, f_y) of x_F, consumed by k_ghost_permute
+    if (!d_gfrac) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the ghost geometry temporaries"); }
     if (c->is32)
       k_ghost_geometry<float><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
                                                      n_disks, d_start, d_list, ncx, kCell, d_smooth, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
-                                                     c->wgt_d, (float*)c->wgt, c->csolid, c->scal + 1);
+                                                     c->wgt_d, (float*)c->wgt, c->csolid, d_gfrac, c->scal + 1);
     else
       k_ghost_geometry<double><<<gb, 128, 0, c->st>>>(ng, c->gidx, prm->nx, prm->ny, prm->wall_rows, d_disks,
                                                       n_disks, d_start, d_list, ncx, kCell, d_smooth, c->cls, c->gnx, c->gny, c->gdepth, c->corner,
-                                                      c->wgt_d, (double*)c->wgt, c->csolid, c->scal + 1);
+                                                      c->wgt_d, (double*)c->wgt, c->csolid, d_gfrac, c->scal + 1);
     CKC(cudaGetLastError());
     int bad = 0;
     cudaMemcpyAsync(&bad, c->scal + 1, sizeof(int), cudaMemcpyDeviceToHost, c->st);
@@ -640,7 +638,6 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
       int *v_in = nullptr, *v_out = nullptr;
       void* tmp = nullptr;
       size_t tmp_bytes = 0;
-      scratch.off = 0;   // the geometry temporaries are done with
       k_in = (unsigned*)scratch_take(4 * sizeof(int) * (size_t)ng);
       if (!k_in) { delete c; return fail(nullptr, LBM_ENOMEM, "workspace too small for the ghost ordering"); }
       cudaError_t e = cudaSuccess;
@@ -651,11 +648,11 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
       if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, k_in, k_out, v_in, v_out, ng, 0, 32, c->st);
       if (e == cudaSuccess) {
         if (c->is32)
-          k_ghost_permute<float><<<(ng + 255) / 256, 256, 0, c->st>>>(ng, v_out, c->gidx, (const int4*)c->corner, (const float*)c->wgt,
-                                                                      c->csolid, c->gidx_p, (int4*)c->corner_p, (float*)c->wgt_p, c->csolid_p);
+          k_ghost_permute<float><<<(ng + 255) / 256, 256, 0, c->st>>>(ng, v_out, c->gidx, (const int4*)c->corner, d_gfrac, c->csolid,
+                                                                      prm->nx, prm->ny, c->gent_p, (float2*)c->gfr_p);
         else
-          k_ghost_permute<double><<<(ng + 255) / 256, 256, 0, c->st>>>(ng, v_out, c->gidx, (const int4*)c->corner, (const double*)c->wgt,
-                                                                       c->csolid, c->gidx_p, (int4*)c->corner_p, (double*)c->wgt_p, c->csolid_p);
+          k_ghost_permute<double><<<(ng + 255) / 256, 256, 0, c->st>>>(ng, v_out, c->gidx, (const int4*)c->corner, d_gfrac, c->csolid,
+                                                                       prm->nx, prm->ny, c->gent_p, (double2*)c->gfr_p);
         e = cudaGetLastError();
       }
       if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);

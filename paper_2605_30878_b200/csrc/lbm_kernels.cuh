@@ -198,7 +198,7 @@ __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __res
                                                         double* __restrict__ gdepth,
                                                         int* __restrict__ corner, double* __restrict__ wgt_d,
                                                         R* __restrict__ wgt, uint8_t* __restrict__ csolid,
-                                                        int* __restrict__ err) {
+                                                        double2* __restrict__ gfrac, int* __restrict__ err) {
   const int g = blockIdx.x * 128 + threadIdx.x;
   if (g >= ng) return;
   const int k = gidx[g];
@@ -265,6 +265,7 @@ __global__ void __launch_bounds__(128) k_ghost_geometry(int ng, const int* __res
   const double w1 = __dmul_rn(fx, __dsub_rn(1.0, fy));
   const double w2 = __dmul_rn(__dsub_rn(1.0, fx), fy);
   const double w3 = __dmul_rn(fx, fy);
+  if (gfrac) gfrac[g] = make_double2(fx, fy);
   corner[4 * g + 0] = c0; corner[4 * g + 1] = c1; corner[4 * g + 2] = c2; corner[4 * g + 3] = c3;
   wgt_d[4 * g + 0] = w0; wgt_d[4 * g + 1] = w1; wgt_d[4 * g + 2] = w2; wgt_d[4 * g + 3] = w3;
   wgt[4 * g + 0] = (R)w0; wgt[4 * g + 1] = (R)w1; wgt[4 * g + 2] = (R)w2; wgt[4 * g + 3] = (R)w3;
@@ -284,20 +285,33 @@ __global__ void __launch_bounds__(256) k_ghost_tile_keys(int ng, const int* __re
   keys[g] = (unsigned)(j >> 5) * (unsigned)((nx + 31) >> 5) + (unsigned)(i >> 5);
   vals[g] = g;
 }
+// The list entry the per-step kernel reads: {node index, code} + (f_x, f_y).  code bits 0-1 / 2-3: i0 - i + 1 and
+// j0 - j + 1 of the interpolation cell's base corner (x_F = x_G + n_s lies within one node of x_G, :66), bits 4-7:
+// corner is a solid node.  The four corner indices and weights follow from it; storing them took 53 B (fp64) per
+// ghost node, this takes 24 B (16 B in fp32).
+template <typename R> struct GhostFrac;
+template <> struct GhostFrac<double> { using T = double2; };
+template <> struct GhostFrac<float> { using T = float2; };
 template <typename R>
 __global__ void __launch_bounds__(256) k_ghost_permute(int ng, const int* __restrict__ perm,
                                                        const int* __restrict__ gidx, const int4* __restrict__ corner,
-                                                       const R* __restrict__ wgt, const uint8_t* __restrict__ csolid,
-                                                       int* __restrict__ gidx_p, int4* __restrict__ corner_p,
-                                                       R* __restrict__ wgt_p, uint8_t* __restrict__ csolid_p) {
+                                                       const double2* __restrict__ gfrac, const uint8_t* __restrict__ csolid,
+                                                       int nx, int ny, uint2* __restrict__ gent_p,
+                                                       typename GhostFrac<R>::T* __restrict__ gfr_p) {
   const int t = blockIdx.x * 256 + threadIdx.x;
   if (t >= ng) return;
   const int g = perm[t];
-  gidx_p[t] = gidx[g];
-  corner_p[t] = corner[g];
-#pragma unroll
-  for (int c = 0; c < 4; c++) wgt_p[4 * t + c] = wgt[4 * g + c];
-  csolid_p[t] = csolid[g];
+  const int k = gidx[g], c0 = corner[g].x;
+  int di = c0 % nx - k % nx, dj = c0 / nx - k / nx;   // base corner relative to the node, periodic
+  if (di > 1) di -= nx;
+  if (di < -1) di += nx;
+  if (dj > 1) dj -= ny;
+  if (dj < -1) dj += ny;
+  gent_p[t] = make_uint2((unsigned)k, (unsigned)(di + 1) | ((unsigned)(dj + 1) << 2) | ((unsigned)csolid[g] << 4));
+  const double2 f = gfrac[g];
+  typename GhostFrac<R>::T o;
+  o.x = (R)f.x; o.y = (R)f.y;
+  gfr_p[t] = o;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -305,25 +319,40 @@ __global__ void __launch_bounds__(256) k_ghost_permute(int ng, const int* __rest
 // x_F = x_G + n_s (:66); Jacobi (R13): fluid corners carry this time's phi (phi_cur), solid
 // corners the previous ghost values (phi_prev; bulk solid nodes are constant in both buffers).
 // ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bilinear_weights(double fx, double fy, double (&w)[4]) {   // as the oracle: no contraction
+  const double gx = __dsub_rn(1.0, fx), gy = __dsub_rn(1.0, fy);
+  w[0] = __dmul_rn(gx, gy); w[1] = __dmul_rn(fx, gy); w[2] = __dmul_rn(gx, fy); w[3] = __dmul_rn(fx, fy);
+}
+__device__ __forceinline__ void bilinear_weights(float fx, float fy, float (&w)[4]) {
+  const float gx = 1.0f - fx, gy = 1.0f - fy;
+  w[0] = gx * gy; w[1] = fx * gy; w[2] = gx * fy; w[3] = fx * fy;
+}
 template <typename R>
 __global__ void __launch_bounds__(128) k_ghost_update(const Consts<R> C, int ng,
-                                                      const int* __restrict__ gidx,
-                                                      const int4* __restrict__ corner,
-                                                      const R* __restrict__ wgt,
-                                                      const uint8_t* __restrict__ csolid,
+                                                      const uint2* __restrict__ gent,
+                                                      const typename GhostFrac<R>::T* __restrict__ gfr,
                                                       const R* __restrict__ phi_prev,
                                                       R* __restrict__ phi_cur) {
   const int g = blockIdx.x * 128 + threadIdx.x;
   if (g >= ng) return;
-  const int4 c = corner[g];
-  const unsigned sb = csolid[g];
-  const R w0 = wgt[4 * g + 0], w1 = wgt[4 * g + 1], w2 = wgt[4 * g + 2], w3 = wgt[4 * g + 3];
-  const R p0 = (sb & 1u) ? phi_prev[c.x] : phi_cur[c.x];
-  const R p1 = (sb & 2u) ? phi_prev[c.y] : phi_cur[c.y];
-  const R p2 = (sb & 4u) ? phi_prev[c.z] : phi_cur[c.z];
-  const R p3 = (sb & 8u) ? phi_prev[c.w] : phi_cur[c.w];
-  const R phiF = ((w0 * p0 + w1 * p1) + w2 * p2) + w3 * p3;
-  phi_cur[gidx[g]] = ghost_rule<R>(C, phiF);
+  const uint2 e = gent[g];
+  const typename GhostFrac<R>::T f = gfr[g];
+  const int nx = C.nx, ny = C.ny;
+  const int k = (int)e.x, i = k % nx, j = k / nx;
+  int i0 = i + (int)(e.y & 3u) - 1, j0 = j + (int)((e.y >> 2) & 3u) - 1;
+  i0 = i0 < 0 ? i0 + nx : (i0 >= nx ? i0 - nx : i0);
+  j0 = j0 < 0 ? j0 + ny : (j0 >= ny ? j0 - ny : j0);
+  const int i1 = i0 + 1 == nx ? 0 : i0 + 1, j1 = j0 + 1 == ny ? 0 : j0 + 1;
+  const int c0 = j0 * nx + i0, c1 = j0 * nx + i1, c2 = j1 * nx + i0, c3 = j1 * nx + i1;
+  const unsigned sb = e.y >> 4;
+  R w[4];
+  bilinear_weights(f.x, f.y, w);
+  const R p0 = (sb & 1u) ? phi_prev[c0] : phi_cur[c0];
+  const R p1 = (sb & 2u) ? phi_prev[c1] : phi_cur[c1];
+  const R p2 = (sb & 4u) ? phi_prev[c2] : phi_cur[c2];
+  const R p3 = (sb & 8u) ? phi_prev[c3] : phi_cur[c3];
+  const R phiF = ((w[0] * p0 + w[1] * p1) + w[2] * p2) + w[3] * p3;
+  phi_cur[k] = ghost_rule<R>(C, phiF);
 }
 
 // ------------------------------------------------------------------------------------------
