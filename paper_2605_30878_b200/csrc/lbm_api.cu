@@ -46,6 +46,7 @@ struct lbm_ctx {
   int fused;
   int sched;         // resolved LBM_SCHEDULE_* (never AUTO)
   int keep_B;
+  int B_owned;       // compacted layouts: the B planes are not in the workspace; lbm_keep_B allocates them on demand
   int B_valid;       // B planes of buffer `cur` hold the post-collision B* of the last step
   cudaStream_t st;
   Consts<double> Cd;
@@ -68,7 +69,6 @@ struct lbm_ctx {
   void* gfr_p;        // (f_x, f_y) in the device precision
   // PACK schedule: pair-compacted population planes (dense N[cur] is a mirror, refreshed on demand)
   int packed;
-  int dense_valid;
   int ccur;
   int nw;            // ptab words per row
   size_t cps;        // compact plane stride in pairs
@@ -228,6 +228,8 @@ long long count_fluid_pairs(const lbm_params* P, const uint8_t* mask) {
   return c;
 }
 
+constexpr size_t kStagePlanes = 3;   // host <-> device staging: nx*ny doubles each (phi0 + u0 of lbm_init is the largest user)
+
 size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long long nfp) {
   const size_t n = (size_t)P->nx * P->ny;
   const size_t rs = P->precision == 32 ? 4 : 8;
@@ -236,11 +238,25 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
   const bool fused = use_fused(P);
   Arena A{base, 0};
   const size_t ps = plane_stride(P);
-  char* N0 = A.take<char>(9 * ps * rs);
-  // compacted planes (PACK / SPARSE) carry the state: one dense mirror is enough (lbm_get, lbm_diag, ... refresh it)
-  char* N1 = use_pack(P) ? nullptr : A.take<char>(9 * ps * rs);
-  char* B0 = A.take<char>(9 * ps * rs);
-  char* B1 = fused ? nullptr : A.take<char>(9 * ps * rs);
+  const int G = pack_group(P->precision == 32 ? 4 : 8, P->nx);
+  const int nw = (P->nx / G + 31) / 32;
+  const size_t cps = (((size_t)(nfp > 0 ? nfp : 1) + 63) & ~(size_t)63) + 37 * 64;
+  // The populations come first (their size does not depend on the ghost count: lbm_create uses them as scratch
+  // before lbm_init).  Compacted layouts (PACK / SPARSE) keep the two compact buffers and NO dense copy: every
+  // call off the hot path reads and writes the compact planes through PopView.  B planes exist in the workspace
+  // only where they are part of the state or of the fall-back kernels (dense layouts).
+  char *N0 = nullptr, *N1 = nullptr, *B0 = nullptr, *B1 = nullptr, *Nc0 = nullptr, *Nc1 = nullptr;
+  uint2* ptab = nullptr;
+  if (use_pack(P)) {
+    Nc0 = A.take<char>(9 * cps * G * rs);
+    Nc1 = A.take<char>(9 * cps * G * rs);
+    ptab = A.take<uint2>((size_t)P->ny * nw);
+  } else {
+    N0 = A.take<char>(9 * ps * rs);
+    N1 = A.take<char>(9 * ps * rs);
+    B0 = A.take<char>(9 * ps * rs);
+    B1 = fused ? nullptr : A.take<char>(9 * ps * rs);
+  }
   char* p0 = A.take<char>(n * rs);
   char* p1 = A.take<char>(n * rs);
   uint8_t* cls = A.take<uint8_t>(n);
@@ -249,7 +265,7 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
   int* blk_cnt = A.take<int>(nblk);
   int* blk_off = A.take<int>(nblk);
   int* scal = A.take<int>(64);
-  double* stage = A.take<double>(5 * n + 64);
+  double* stage = A.take<double>(kStagePlanes * n + 64);
   double* diag_out = A.take<double>(8);
   const size_t samp_cap = 1 << 20;
   long long* samp = A.take<long long>(samp_cap);
@@ -263,17 +279,6 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
   uint8_t* csolid = A.take<uint8_t>(g);
   uint2* gent_p = A.take<uint2>(g);
   char* gfr_p = A.take<char>(2 * g * rs);
-  // PACK schedule (last, so that nothing above depends on the pair count)
-  uint2* ptab = nullptr;
-  char *Nc0 = nullptr, *Nc1 = nullptr;
-  const int G = pack_group(P->precision == 32 ? 4 : 8, P->nx);
-  const int nw = (P->nx / G + 31) / 32;
-  const size_t cps = (((size_t)(nfp > 0 ? nfp : 1) + 63) & ~(size_t)63) + 37 * 64;
-  if (use_pack(P)) {
-    ptab = A.take<uint2>((size_t)P->ny * nw);
-    Nc0 = A.take<char>(9 * cps * G * rs);
-    Nc1 = A.take<char>(9 * cps * G * rs);
-  }
   SpDesc* sp_desc = nullptr; uint16_t* sp_cnt = nullptr; uint2* sp_meta = nullptr; SpMarch* sp_march = nullptr; int* sp_first = nullptr;
   if (use_sparse(P)) {
     const size_t nsr = (size_t)sp_strips(P) * P->ny;
@@ -373,14 +378,12 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
       done = launch_fused_sparse(c, C, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po);
       if (!done) return LBM_ECUDA;
       c->ccur ^= 1;
-      c->dense_valid = 0;
       c->cur ^= 1;     // undone below: the dense buffer index does not move
     } else if (c->packed) {   // PACK: compact planes step compact -> compact; the dense mirror N[cur] goes stale
       done = launch_fused_pack(C, c->cl16, (const R*)c->Nc[c->ccur], (R*)c->Nc[c->ccur ^ 1], Bd, pi, po, c->st, c->ptab,
                                c->nw, (unsigned)(c->cps * pack_group((int)sizeof(R), c->P.nx) * sizeof(R)));
       if (!done) return LBM_ECUDA;   // never step the stale dense mirror instead
       c->ccur ^= 1;
-      c->dense_valid = 0;
       c->cur ^= 1;     // undone below: the dense buffer index does not move
     }
     if (!done && c->sched == LBM_SCHEDULE_PAIR) done = launch_fused_pair(C, c->cl16, Ns, Nd, Bd, pi, po, c->st);   // false: odd nx
@@ -450,23 +453,18 @@ void sp_partition(const uint16_t* cnt, int nstrips, int ny, int ncta_max, std::v
   while (cur < ncta) { first.push_back((int)marches.size()); cur++; }
 }
 
-// PACK schedule: refresh the dense mirror N[cur] from the compact planes before a dense reader runs
-void ensure_dense(lbm_ctx* c) {
-  if (!c->packed || c->dense_valid) return;
-  const int G = pack_group(c->is32 ? 4 : 8, c->P.nx);
-  const long long np = (long long)c->P.ny * (c->P.nx / G);
-  const unsigned nb = (unsigned)((np + 255) / 256);
-  if (c->is32)
-    k_pair_repack<float, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, G, c->Cf.ps, c->cps,
-                                                       (float*)c->N[c->cur], (float*)c->Nc[c->ccur], c->sparse);
-  else
-    k_pair_repack<double, false><<<nb, 256, 0, c->st>>>(c->ptab, c->P.nx, c->P.ny, c->nw, G, c->Cd.ps, c->cps,
-                                                        (double*)c->N[c->cur], (double*)c->Nc[c->ccur], c->sparse);
-  c->launches[3]++;
-  c->dense_valid = 1;
+// the populations of the current time, wherever they live (dense planes or the compact buffers of PACK / SPARSE)
+template <typename R>
+PopView<R> pop_view(const lbm_ctx* c) {
+  if (c->packed)
+    return PopView<R>{(R*)c->Nc[c->ccur], 0, c->ptab, c->P.nx, c->nw, pack_group((int)sizeof(R), c->P.nx), c->sparse, c->cps};
+  return dense_view<R>((R*)c->N[c->cur], plane_stride(&c->P), c->P.nx);
+}
+template <typename R>
+PopView<R> B_view(const lbm_ctx* c) {
+  return dense_view<R>((R*)(c->fused ? c->B[0] : c->B[c->cur]), plane_stride(&c->P), c->P.nx);
 }
 
-const void* B_planes(const lbm_ctx* c) { return c->fused ? c->B[0] : c->B[c->cur]; }
 
 }  // namespace
 
@@ -553,8 +551,10 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   } while (0)
 
   // temporaries of this call are carved from the dense population planes, which hold nothing before lbm_init
-  Arena scratch{(char*)c->N[0], 0};
-  const size_t scratch_cap = 9 * plane_stride(prm) * (size_t)(c->is32 ? 4 : 8);
+  Arena scratch{(char*)(c->Nc[0] ? c->Nc[0] : c->N[0]), 0};
+  const size_t rs_ = c->is32 ? 4 : 8;
+  const size_t scratch_cap = c->Nc[0] ? 2 * 9 * c->cps * (size_t)pack_group((int)rs_, prm->nx) * rs_   // both compact buffers
+                                      : 2 * 9 * plane_stride(prm) * rs_;                               // both dense buffers
   auto scratch_take = [&](size_t bytes) -> void* {
     char* p0 = scratch.take<char>(bytes);
     return scratch.off <= scratch_cap ? p0 : nullptr;
@@ -584,7 +584,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     k_compact_ghosts<<<nblk, 256, 0, c->st>>>(c->cls, (long long)n, c->blk_off, c->gidx);
     // disk list staged behind the mask copy in the stage area (5n doubles >= n bytes + disks?)
     const size_t disk_bytes = (size_t)n_disks * sizeof(Disk);
-    const size_t stage_bytes = (5 * n + 64) * sizeof(double);
+    const size_t stage_bytes = (kStagePlanes * n + 64) * sizeof(double);
     const size_t disk_off = (n + 255) & ~(size_t)255;
     if (disk_off + disk_bytes > stage_bytes) {
       delete c;
@@ -726,6 +726,7 @@ void lbm_destroy(lbm_ctx* ctx) {
   if (!ctx) return;
   for (auto& g : ctx->gexec)
     if (g) cudaGraphExecDestroy(g);
+  if (ctx->B_owned) cudaFree(ctx->B[0]);
   delete ctx;
 }
 
@@ -741,28 +742,16 @@ int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
   ctx->t = 0;
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
-  void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];
+  ctx->ccur = 0;
+  void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];   // may be absent (compacted layout without lbm_keep_B)
   if (ctx->is32)
-    k_init<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, d_phi0, d_u0, (float*)ctx->N[0],
+    k_init<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, d_phi0, d_u0, pop_view<float>(ctx),
                                             (float*)Bp, (float*)ctx->phi[0], (float*)ctx->phi[1]);
   else
-    k_init<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, d_phi0, d_u0, (double*)ctx->N[0],
+    k_init<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, d_phi0, d_u0, pop_view<double>(ctx),
                                              (double*)Bp, (double*)ctx->phi[0], (double*)ctx->phi[1]);
   ctx->launches[3]++;
-  ctx->B_valid = 1;
-  if (ctx->packed) {   // PACK: the compact planes start as a copy of the dense initial state
-    const int G = pack_group(ctx->is32 ? 4 : 8, ctx->P.nx);
-    const long long np = (long long)ctx->P.ny * (ctx->P.nx / G);
-    const unsigned nb = (unsigned)((np + 255) / 256);
-    if (ctx->is32)
-      k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cf.ps, ctx->cps,
-                                                          (float*)ctx->N[0], (float*)ctx->Nc[0], ctx->sparse);
-    else
-      k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cd.ps, ctx->cps,
-                                                           (double*)ctx->N[0], (double*)ctx->Nc[0], ctx->sparse);
-    ctx->ccur = 0;
-    ctx->dense_valid = 1;
-  }
+  ctx->B_valid = Bp ? 1 : 0;
   if (ctx->is32) launch_ghost<float>(ctx); else launch_ghost<double>(ctx);
   CK(cudaGetLastError());
   CK(cudaStreamSynchronize(ctx->st));
@@ -809,7 +798,6 @@ int lbm_step(lbm_ctx* ctx, int64_t nsteps) {
         ctx->t += kGraphSteps;
         for (int k = 0; k < 4; k++) ctx->launches[k] += ctx->gdelta[key][k];
         ctx->B_valid = ctx->fused ? 0 : 1;
-        if (ctx->packed) ctx->dense_valid = 0;
       }
       CK(cudaGraphLaunch(ctx->gexec[key], ctx->st));
       s += kGraphSteps;
@@ -867,36 +855,51 @@ int lbm_sync(lbm_ctx* ctx) {
 
 int lbm_keep_B(lbm_ctx* ctx, int32_t on) {
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
+  if (on && ctx->fused && !ctx->B[0]) {   // compacted layouts carry no B planes in the workspace: allocate them now
+    const size_t bytes = 9 * plane_stride(&ctx->P) * (size_t)(ctx->is32 ? 4 : 8);
+    void* b = nullptr;
+    CK(cudaMalloc(&b, bytes));
+    CK(cudaMemsetAsync(b, 0, bytes, ctx->st));
+    ctx->B[0] = b;
+    ctx->B_owned = 1;
+    ctx->B_valid = 0;
+  }
   ctx->keep_B = on ? 1 : 0;
   return LBM_OK;
 }
 
 int lbm_get(lbm_ctx* ctx, double* rho, double* phi, double* ux, double* uy, double* p) {
-  if (ctx) ensure_dense(ctx);
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   const size_t n = ctx->n;
-  double* s = ctx->stage;
-  double* d[5] = {rho ? s : nullptr, phi ? s + n : nullptr, ux ? s + 2 * n : nullptr,
-                  uy ? s + 3 * n : nullptr, p ? s + 4 * n : nullptr};
   double* h[5] = {rho, phi, ux, uy, p};
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
-  if (ctx->is32)
-    k_moments<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)ctx->N[ctx->cur],
-                                               (const float*)ctx->phi[ctx->pcur], d[0], d[1], d[2], d[3], d[4]);
-  else
-    k_moments<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)ctx->N[ctx->cur],
-                                                (const double*)ctx->phi[ctx->pcur], d[0], d[1], d[2], d[3], d[4]);
-  ctx->launches[3]++;
-  CK(cudaGetLastError());
-  for (int f = 0; f < 5; f++)
-    if (h[f]) CK(cudaMemcpyAsync(h[f], d[f], n * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
-  CK(cudaStreamSynchronize(ctx->st));
+  // the moments kernel writes the fields it is given; the staging area holds kStagePlanes of them at a time
+  int f = 0;
+  while (f < 5) {
+    double* d[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    int used = 0, f1 = f;
+    for (; f1 < 5 && used < (int)kStagePlanes; f1++)
+      if (h[f1]) d[f1] = ctx->stage + (size_t)(used++) * n;
+    if (used) {
+      if (ctx->is32)
+        k_moments<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, pop_view<float>(ctx),
+                                                   (const float*)ctx->phi[ctx->pcur], d[0], d[1], d[2], d[3], d[4]);
+      else
+        k_moments<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, pop_view<double>(ctx),
+                                                    (const double*)ctx->phi[ctx->pcur], d[0], d[1], d[2], d[3], d[4]);
+      ctx->launches[3]++;
+      CK(cudaGetLastError());
+      for (int k = f; k < f1; k++)
+        if (d[k]) CK(cudaMemcpyAsync(h[k], d[k], n * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+      CK(cudaStreamSynchronize(ctx->st));
+    }
+    f = f1;
+  }
   return LBM_OK;
 }
 
 int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
-  if (ctx) ensure_dense(ctx);
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   if (B && !ctx->B_valid)
     return fail(ctx, LBM_EINVAL, "B is not stored under this schedule: call lbm_keep_B(ctx, 1) before lbm_step");
@@ -908,16 +911,16 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
   for (int which = 0; which < 2; which++) {
     double* host = which ? B : N;
     if (!host) continue;
-    const void* pop = which ? B_planes(ctx) : ctx->N[ctx->cur];
-    for (int q0 = 0; q0 < 9; q0 += 5) {          // 5 staging planes at a time
-      const int q1 = q0 + 5 < 9 ? q0 + 5 : 9;
+    const int CH = (int)kStagePlanes;             // staging planes at a time
+    for (int q0 = 0; q0 < 9; q0 += CH) {
+      const int q1 = q0 + CH < 9 ? q0 + CH : 9;
       for (int q = q0; q < q1; q++) {
         double* dst = ctx->stage + (size_t)(q - q0) * n;
         const double add = which ? 0.0 : chi[q];
         if (ctx->is32)
-          k_gather_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)pop, q, add, dst);
+          k_gather_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, which ? B_view<float>(ctx) : pop_view<float>(ctx), q, add, dst);
         else
-          k_gather_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)pop, q, add, dst);
+          k_gather_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, which ? B_view<double>(ctx) : pop_view<double>(ctx), q, add, dst);
         ctx->launches[3]++;
       }
       CK(cudaGetLastError());
@@ -932,29 +935,29 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
 int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B) {
   if (!ctx) return fail(ctx, LBM_EINVAL, "null context");
   if (!N && !B) return LBM_OK;
-  ensure_dense(ctx);   // planes that are not given keep their values
   const size_t n = ctx->n;
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
   const double chi[9] = {ctx->Cd.chi0, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1,
                          ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5};
-  void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];
-  double* acc = ctx->stage + 4 * n;   // planes 0..3 stage the input, plane 4 accumulates phi
+  void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];   // may be absent (compacted layout without lbm_keep_B)
+  const int CH = (int)kStagePlanes - 1;                    // planes 0 .. CH-1 stage the input, the last one accumulates phi
+  double* acc = ctx->stage + (size_t)CH * n;
   for (int which = 0; which < 2; which++) {
     const double* host = which ? B : N;
     if (!host) continue;
-    void* pop = which ? Bp : ctx->N[ctx->cur];
-    for (int q0 = 0; q0 < 9; q0 += 4) {
-      const int q1 = q0 + 4 < 9 ? q0 + 4 : 9;
+    const bool scatter = which ? Bp != nullptr : true;
+    for (int q0 = 0; q0 < 9; q0 += CH) {
+      const int q1 = q0 + CH < 9 ? q0 + CH : 9;
       CK(cudaMemcpyAsync(ctx->stage, host + (size_t)q0 * n, (size_t)(q1 - q0) * n * sizeof(double), cudaMemcpyHostToDevice, ctx->st));
       for (int q = q0; q < q1; q++) {
         const double* src = ctx->stage + (size_t)(q - q0) * n;
         const double sub = which ? 0.0 : chi[q];
         if (ctx->is32) {
-          if (pop) k_scatter_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, src, q, sub, (float*)pop);
+          if (scatter) k_scatter_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, src, q, sub, which ? B_view<float>(ctx) : pop_view<float>(ctx));
           if (which) k_phi_accumulate<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, src, q == 0, acc, q == 8 ? (float*)ctx->phi[ctx->pcur] : nullptr);
         } else {
-          if (pop) k_scatter_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, src, q, sub, (double*)pop);
+          if (scatter) k_scatter_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, src, q, sub, which ? B_view<double>(ctx) : pop_view<double>(ctx));
           if (which) k_phi_accumulate<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, src, q == 0, acc, q == 8 ? (double*)ctx->phi[ctx->pcur] : nullptr);
         }
         ctx->launches[3] += which ? 2 : 1;
@@ -962,18 +965,6 @@ int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B) {
       CK(cudaGetLastError());
       CK(cudaStreamSynchronize(ctx->st));   // the staging planes are reused by the next chunk
     }
-  }
-  if (N && ctx->packed) {   // the compact planes follow the dense ones
-    const int G = pack_group(ctx->is32 ? 4 : 8, ctx->P.nx);
-    const long long np = (long long)ctx->P.ny * (ctx->P.nx / G);
-    const unsigned nb = (unsigned)((np + 255) / 256);
-    if (ctx->is32)
-      k_pair_repack<float, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cf.ps, ctx->cps,
-                                                          (float*)ctx->N[ctx->cur], (float*)ctx->Nc[ctx->ccur], ctx->sparse);
-    else
-      k_pair_repack<double, true><<<nb, 256, 0, ctx->st>>>(ctx->ptab, ctx->P.nx, ctx->P.ny, ctx->nw, G, ctx->Cd.ps, ctx->cps,
-                                                           (double*)ctx->N[ctx->cur], (double*)ctx->Nc[ctx->ccur], ctx->sparse);
-    ctx->launches[3]++;
   }
   if (B) {
     ctx->B_valid = Bp ? 1 : 0;
@@ -985,30 +976,33 @@ int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B) {
 }
 
 int lbm_sample_populations(lbm_ctx* ctx, int64_t n_idx, const int64_t* idx, double* N, double* B) {
-  if (ctx) ensure_dense(ctx);
   if (!ctx || n_idx < 0 || (n_idx > 0 && !idx)) return fail(ctx, LBM_EINVAL, "bad argument");
   if (B && !ctx->B_valid)
     return fail(ctx, LBM_EINVAL, "B is not stored under this schedule: call lbm_keep_B(ctx, 1) before lbm_step");
-  if ((size_t)n_idx > ctx->samp_cap || (size_t)n_idx * 9 > 5 * ctx->n) return fail(ctx, LBM_EINVAL, "too many samples");
   for (int64_t t = 0; t < n_idx; t++)
     if (idx[t] < 0 || (size_t)idx[t] >= ctx->n) return fail(ctx, LBM_EINVAL, "sample index out of range");
-  if (n_idx == 0) return LBM_OK;
-  CK(cudaMemcpyAsync(ctx->samp_idx, idx, (size_t)n_idx * sizeof(long long), cudaMemcpyHostToDevice, ctx->st));
-  const unsigned gb = (unsigned)((n_idx + 127) / 128);
-  for (int which = 0; which < 2; which++) {
-    double* host = which ? B : N;
-    if (!host) continue;
-    const void* pop = which ? B_planes(ctx) : ctx->N[ctx->cur];
-    if (ctx->is32)
-      k_gather_samples<float><<<gb, 128, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)pop, which ? 0 : 1,
-                                                       (long long)n_idx, ctx->samp_idx, ctx->stage);
-    else
-      k_gather_samples<double><<<gb, 128, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)pop, which ? 0 : 1,
-                                                        (long long)n_idx, ctx->samp_idx, ctx->stage);
-    ctx->launches[3]++;
-    CK(cudaGetLastError());
-    CK(cudaMemcpyAsync(host, ctx->stage, (size_t)n_idx * 9 * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
-    CK(cudaStreamSynchronize(ctx->st));
+  // chunks sized by the index buffer and by the staging area (9 doubles per sample)
+  const int64_t chunk = (int64_t)std::min<size_t>(ctx->samp_cap, std::max<size_t>(1, kStagePlanes * ctx->n / 9));
+  for (int64_t t0 = 0; t0 < n_idx; t0 += chunk) {
+    const int64_t m = std::min<int64_t>(chunk, n_idx - t0);
+    CK(cudaMemcpyAsync(ctx->samp_idx, idx + t0, (size_t)m * sizeof(long long), cudaMemcpyHostToDevice, ctx->st));
+    const unsigned gb = (unsigned)((m + 127) / 128);
+    for (int which = 0; which < 2; which++) {
+      double* host = which ? B : N;
+      if (!host) continue;
+      if (ctx->is32)
+        k_gather_samples<float><<<gb, 128, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, which ? B_view<float>(ctx) : pop_view<float>(ctx),
+                                                         which ? 0 : 1, (long long)m, ctx->samp_idx, ctx->stage);
+      else
+        k_gather_samples<double><<<gb, 128, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, which ? B_view<double>(ctx) : pop_view<double>(ctx),
+                                                          which ? 0 : 1, (long long)m, ctx->samp_idx, ctx->stage);
+      ctx->launches[3]++;
+      CK(cudaGetLastError());
+      // device [q][m] -> host [q][n_idx] at column t0
+      CK(cudaMemcpy2DAsync(host + t0, (size_t)n_idx * sizeof(double), ctx->stage, (size_t)m * sizeof(double),
+                           (size_t)m * sizeof(double), 9, cudaMemcpyDeviceToHost, ctx->st));
+      CK(cudaStreamSynchronize(ctx->st));
+    }
   }
   return LBM_OK;
 }
@@ -1033,18 +1027,17 @@ int lbm_get_classification(lbm_ctx* ctx, uint8_t* cls, int32_t* n_ghost, int32_t
 }
 
 int lbm_diag(lbm_ctx* ctx, double out[8]) {
-  if (ctx) ensure_dense(ctx);
   if (!ctx || !out) return fail(ctx, LBM_EINVAL, "null argument");
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
   const long long m = (long long)grid.x * grid.y;
-  if ((size_t)m * sizeof(DiagVec) > (5 * ctx->n + 64) * sizeof(double)) return fail(ctx, LBM_EINVAL, "grid too small for diag staging");
+  if ((size_t)m * sizeof(DiagVec) > (kStagePlanes * ctx->n + 64) * sizeof(double)) return fail(ctx, LBM_EINVAL, "grid too small for diag staging");
   DiagVec* part = reinterpret_cast<DiagVec*>(ctx->stage);
   if (ctx->is32)
-    k_diag_partial<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, (const float*)ctx->N[ctx->cur],
+    k_diag_partial<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, pop_view<float>(ctx),
                                                     (const float*)ctx->phi[ctx->pcur], part);
   else
-    k_diag_partial<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, (const double*)ctx->N[ctx->cur],
+    k_diag_partial<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, pop_view<double>(ctx),
                                                      (const double*)ctx->phi[ctx->pcur], part);
   k_diag_final<<<1, 1024, 0, ctx->st>>>(part, m, ctx->diag_out);
   ctx->launches[3] += 2;
@@ -1055,17 +1048,13 @@ int lbm_diag(lbm_ctx* ctx, double out[8]) {
 }
 
 int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass) {
-  if (ctx) ensure_dense(ctx);
   if (!ctx || iters < 1 || !ms_per_pass) return fail(ctx, LBM_EINVAL, "bad argument");
+  if (ctx->packed) return fail(ctx, LBM_EINVAL, "the dense SoA layout this helper measures is not kept under PACK / SPARSE; create the context with LBM_SCHEDULE_PAIR");
   const size_t rs = ctx->is32 ? 4 : 8, nps = 32 / rs;
   if (ctx->n % nps != 0 || ctx->Cd.ps % nps != 0) return fail(ctx, LBM_EINVAL, "nx*ny is not a whole number of 32-byte sectors");
   const size_t nsec = ctx->n / nps, psec = ctx->Cd.ps / nps;
   const float4* src = (const float4*)ctx->N[ctx->cur];
   float4* dst = (float4*)ctx->N[ctx->cur ^ 1];          // scratch: the next step overwrites it
-  if (!dst) {                                            // compacted state: no second dense buffer, the B planes serve
-    dst = (float4*)ctx->B[0];
-    ctx->B_valid = 0;
-  }
   const float4* psrc = (const float4*)ctx->phi[ctx->pcur];
   float4* pdst = (float4*)ctx->stage;                    // scratch (phi[pcur ^ 1] holds the previous ghost values)
   cudaEvent_t e0, e1;

@@ -358,6 +358,41 @@ __global__ void __launch_bounds__(128) k_ghost_update(const Consts<R> C, int ng,
 // ------------------------------------------------------------------------------------------
 // pulled (post-stream) population q of node k: propagation A16-A17 + half-way bounce-back (R12)
 // ------------------------------------------------------------------------------------------
+// Where a set of nine population planes lives: dense (pop[q * ps + idx]) or group-compacted (PACK / SPARSE, see
+// k_pair_mask below).  The fused kernels address their layout directly; everything off the hot path (lbm_init,
+// lbm_get, lbm_diag, lbm_get/set_populations) goes through this view, so that a compacted context needs no dense
+// copy of its state.
+template <typename R>
+struct PopView {
+  R* base;
+  size_t ps;            // dense: element stride between planes
+  const uint2* ptab;    // nullptr: dense
+  int nx, nw, G, group_major;
+  size_t cps;
+  __device__ __forceinline__ bool has(int idx) const {   // storage exists for this node (its group holds a fluid node)
+    if (!ptab) return true;
+    const int j = idx / nx, p = (idx - j * nx) / G;
+    return (ptab[(size_t)j * nw + (p >> 5)].x >> (p & 31)) & 1u;
+  }
+  __device__ __forceinline__ size_t off(int q, int idx) const {
+    if (!ptab) return (size_t)q * ps + (size_t)idx;
+    const int j = idx / nx, i = idx - j * nx, p = i / G;
+    const uint2 tb = ptab[(size_t)j * nw + (p >> 5)];
+    const size_t ci = (size_t)tb.y + (size_t)__popc(tb.x & ((1u << (p & 31)) - 1u));
+    return group_major ? (ci * 9 + (size_t)q) * G + (size_t)(i - p * G) : ((size_t)q * cps + ci) * G + (size_t)(i - p * G);
+  }
+  __device__ __forceinline__ R& at(int q, int idx) const { return base[off(q, idx)]; }
+};
+template <typename R>
+inline PopView<R> dense_view(R* base, size_t ps, int nx) { return PopView<R>{base, ps, nullptr, nx, 0, 1, 0, 0}; }
+
+template <typename R>
+__device__ __forceinline__ void pull9(const PopView<R>& P, int k, const Nbr& b, unsigned lk, R (&v)[9]) {
+  v[0] = P.at(0, k);
+#pragma unroll
+  for (int q = 1; q < 9; q++) v[q] = ((lk >> (q - 1)) & 1u) ? P.at(opp(q), k) : P.at(q, b.src[q]);
+}
+
 template <typename R>
 __device__ __forceinline__ void pull9(const R* __restrict__ pop, size_t n, int k, const Nbr& b,
                                       unsigned lk, R (&v)[9]) {
@@ -449,7 +484,7 @@ template <typename R>
 __global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* __restrict__ cls,
                                               const uint8_t* __restrict__ links,
                                               const double* __restrict__ phi0,
-                                              const double* __restrict__ u0, R* __restrict__ Npop,
+                                              const double* __restrict__ u0, const PopView<R> Npop,
                                               R* __restrict__ Bpop, R* __restrict__ phiA,
                                               R* __restrict__ phiB) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
@@ -460,9 +495,10 @@ __global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* 
   if (c >= 2) {
     phiA[k] = C.phi_solid;
     phiB[k] = C.phi_solid;
+    const bool stored = Npop.has(k);   // a solid node travels with its group only if the group holds a fluid node
 #pragma unroll
     for (int q = 0; q < 9; q++) {
-      Npop[q * n + k] = R(0);
+      if (stored) Npop.at(q, k) = R(0);
       if (Bpop) Bpop[q * n + k] = R(0);
     }
     return;
@@ -480,7 +516,7 @@ __global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* 
     const int qq = blocked ? oq : q;
     const R ux = u0 ? (R)u0[src] : R(0), uy = u0 ? (R)u0[(size_t)C.nx * C.ny + src] : R(0);
     const R dev = neq_dev_p0<R>(qq, ux, uy);
-    Npop[q * n + k] = dev;
+    Npop.at(q, k) = dev;
     if (Bpop) Bpop[q * n + k] = (R)phi0[src] * (chi[qq] + dev);
     // phi(x, 0) = sum_i B_i(x, 0) = sum_i phi0(x) N_i^eq(u0(x)) in the oracle's order (A13)
     const R uxk = u0 ? (R)u0[k] : R(0), uyk = u0 ? (R)u0[(size_t)C.nx * C.ny + k] : R(0);
@@ -496,7 +532,7 @@ __global__ void __launch_bounds__(256) k_init(const Consts<R> C, const uint8_t* 
 template <typename R>
 __global__ void __launch_bounds__(256) k_moments(const Consts<R> C, const uint8_t* __restrict__ cls,
                                                  const uint8_t* __restrict__ links,
-                                                 const R* __restrict__ Nsrc, const R* __restrict__ phi,
+                                                 const PopView<R> Nsrc, const R* __restrict__ phi,
                                                  double* __restrict__ o_rho, double* __restrict__ o_phi,
                                                  double* __restrict__ o_ux, double* __restrict__ o_uy,
                                                  double* __restrict__ o_p) {
@@ -518,7 +554,7 @@ __global__ void __launch_bounds__(256) k_moments(const Consts<R> C, const uint8_
   R nn[9], ph[9], ns[9], bs[9];
   NodeOut<R> o;
   load_phi9<R>(phi, b, ph);
-  pull9<R>(Nsrc, n, k, b, lk, nn);
+  pull9<R>(Nsrc, k, b, lk, nn);
   node_update<R, false>(C, nn, ph, ns, bs, &o);
   if (o_rho) o_rho[k] = (double)o.rho;
   if (o_ux) o_ux[k] = (double)o.ux;
@@ -530,7 +566,7 @@ __global__ void __launch_bounds__(256) k_moments(const Consts<R> C, const uint8_
 template <typename R>
 __global__ void __launch_bounds__(256) k_gather_plane(const Consts<R> C, const uint8_t* __restrict__ cls,
                                                       const uint8_t* __restrict__ links,
-                                                      const R* __restrict__ pop, int q, double add,
+                                                      const PopView<R> pop, int q, double add,
                                                       double* __restrict__ out) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
@@ -541,8 +577,8 @@ __global__ void __launch_bounds__(256) k_gather_plane(const Consts<R> C, const u
   const Nbr b = make_nbr(i, j, C.nx, C.ny);
   const unsigned lk = (c == 1) ? links[k] : 0u;
   R v;
-  if (q == 0) v = pop[k];
-  else v = ((lk >> (q - 1)) & 1u) ? pop[opp(q) * n + k] : pop[q * n + b.src[q]];
+  if (q == 0) v = pop.at(0, k);
+  else v = ((lk >> (q - 1)) & 1u) ? pop.at(opp(q), k) : pop.at(q, b.src[q]);
   out[k] = (double)v + add;
 }
 
@@ -553,7 +589,7 @@ template <typename R>
 __global__ void __launch_bounds__(256) k_scatter_plane(const Consts<R> C, const uint8_t* __restrict__ cls,
                                                        const uint8_t* __restrict__ links,
                                                        const double* __restrict__ in, int q, double sub,
-                                                       R* __restrict__ pop) {
+                                                       const PopView<R> pop) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (i >= C.nx) return;
   const size_t n = C.ps;   // plane stride
@@ -563,9 +599,9 @@ __global__ void __launch_bounds__(256) k_scatter_plane(const Consts<R> C, const 
   const Nbr b = make_nbr(i, j, C.nx, C.ny);
   const unsigned lk = (c == 1) ? links[k] : 0u;
   const R v = (R)(in[k] - sub);
-  if (q == 0) pop[k] = v;
-  else if ((lk >> (q - 1)) & 1u) pop[opp(q) * n + k] = v;
-  else pop[q * n + b.src[q]] = v;
+  if (q == 0) pop.at(0, k) = v;
+  else if ((lk >> (q - 1)) & 1u) pop.at(opp(q), k) = v;
+  else pop.at(q, b.src[q]) = v;
 }
 // phi = sum_q B_q on fluid nodes (A13, :311), accumulated plane by plane in the oracle's order q = 0 .. 8
 template <typename R>
@@ -585,7 +621,7 @@ __global__ void __launch_bounds__(256) k_phi_accumulate(const Consts<R> C, const
 template <typename R>
 __global__ void __launch_bounds__(128) k_gather_samples(const Consts<R> C, const uint8_t* __restrict__ cls,
                                                         const uint8_t* __restrict__ links,
-                                                        const R* __restrict__ pop, int add_chi,
+                                                        const PopView<R> pop, int add_chi,
                                                         long long m, const long long* __restrict__ idx,
                                                         double* __restrict__ out) {
   const long long t = (long long)blockIdx.x * 128 + threadIdx.x;
@@ -601,8 +637,8 @@ __global__ void __launch_bounds__(128) k_gather_samples(const Consts<R> C, const
     double v = 0.0;
     if (c < 2) {
       R x;
-      if (q == 0) x = pop[k];
-      else x = ((lk >> (q - 1)) & 1u) ? pop[opp(q) * n + k] : pop[q * n + b.src[q]];
+      if (q == 0) x = pop.at(0, k);
+      else x = ((lk >> (q - 1)) & 1u) ? pop.at(opp(q), k) : pop.at(q, b.src[q]);
       v = (double)x + (add_chi ? chi[q] : 0.0);
     }
     out[q * m + t] = v;
@@ -654,7 +690,7 @@ __device__ __forceinline__ DiagVec diag_block_reduce(DiagVec v, DiagVec* sh) {
 template <typename R>
 __global__ void __launch_bounds__(256) k_diag_partial(const Consts<R> C, const uint8_t* __restrict__ cls,
                                                       const uint8_t* __restrict__ links,
-                                                      const R* __restrict__ Nsrc, const R* __restrict__ phi,
+                                                      const PopView<R> Nsrc, const R* __restrict__ phi,
                                                       DiagVec* __restrict__ partial) {
   __shared__ DiagVec sh[32];
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
@@ -669,7 +705,7 @@ __global__ void __launch_bounds__(256) k_diag_partial(const Consts<R> C, const u
       R nn[9], ph[9], ns[9], bs[9];
       NodeOut<R> o;
       load_phi9<R>(phi, b, ph);
-      pull9<R>(Nsrc, n, k, b, lk, nn);
+      pull9<R>(Nsrc, k, b, lk, nn);
       node_update<R, false>(C, nn, ph, ns, bs, &o);
       const double f = (double)ph[0], ux = (double)o.ux, uy = (double)o.uy;
       const double u2 = ux * ux + uy * uy;

@@ -114,6 +114,7 @@ def test_classification_configs_bit_exact(make):
 def test_init_and_first_ghost_update(schedule):
     w = wl.config1(seed=2)
     g, o = make_pair(w, schedule=schedule)
+    g.keep_B(True)                                      # B_i are not part of the stored state (compacted layouts: no B planes at all)
     g.init(w.phi0); o.init(w.phi0)
     fluid = w.mask == 0
     eN, eB = pop_errors(g, o, fluid)
@@ -431,6 +432,37 @@ def test_config5_8192_windows_against_oracle(precision):
     g.close()
 
 
+def test_config5_16384_fp64_on_one_gpu():
+    """Compacted layouts keep no dense copy of the state (workspace 9.8 GB at 8192^2 fp64, 39 GB at 16384^2):
+    the 16384^2 fp64 domain runs on one B200.  Mass is conserved and a window of it, past every 32-bit element
+    offset of a dense plane, agrees with the oracle run on that window."""
+    from oracle import ref
+    from paper_2605_30878_b200 import binding
+    n, steps, size = 16384, 3, 400
+    w = wl.config5(seed=0, n=n)
+    g = binding.LBM(binding.LBMParams(precision=64, **w.param_dict()), w.mask, w.disks)
+    assert g.workspace_bytes < 45e9
+    g.init(w.phi0)
+    m0 = g.diag()["sum_phi"]
+    g.step(steps)
+    d = g.diag()
+    assert d["nan"] == 0 and abs(d["sum_phi"] - m0) <= 1e-11 * m0
+    G = g.get(fields=("phi", "ux", "uy"))
+    h = 4 * steps + 2 + 68
+    x0, y0 = n - 200, n - 200                                  # across both periodic seams, last rows and columns
+    ww, jj, ii = _window_case(w, x0, y0, size)
+    o = ref.RefLBM(ref.RefParams(**ww.param_dict()), ww.mask, ww.disks)
+    o.init(ww.phi0); o.step(steps)
+    O = o.get()
+    inner = np.zeros((size, size), bool); inner[h:-h, h:-h] = True
+    for k in ("phi", "ux", "uy"):
+        assert np.abs(G[k][jj, ii] - O[k])[inner].max() <= 1e-12, k
+    fl = inner & (ww.mask == 0)
+    idx = (jj.astype(np.int64) * n + ii)[fl]
+    assert np.abs(g.sample_populations(idx)[0] - o.get_populations()[0][:, fl]).max() <= 1e-13
+    g.close()
+
+
 def test_config5_8192_is_deterministic():
     """Two runs of the 8192^2 AUTO schedule, 200 steps each, give bit-identical phi and sampled populations:
     the evidence against races in the warp-private rings that is available while compute-sanitizer is closed
@@ -463,14 +495,21 @@ def test_set_populations_round_trip_and_restart(schedule):
     N2 = No * (1.0 + 0.05 * rng.standard_normal(No.shape))        # 5 % noise: far from equilibrium
     B2 = N2 * np.clip(Bo / np.maximum(No, 1e-300) + 0.1 * rng.standard_normal(No.shape), 0.0, 1.0)
     N2[:, ~fluid] = 0.0; B2[:, ~fluid] = 0.0
+    g.keep_B(True)
     g.set_populations(N2, B2); o.set_populations(N2, B2)
     Ng, Bg = g.get_populations(want_B=True)
     assert np.abs(Ng - N2)[:, fluid].max() <= 1e-15 and np.abs(Bg - B2)[:, fluid].max() <= 1e-15
-    g.keep_B(True)
     g.step(3); o.step(3)
     eN, eB = pop_errors(g, o, fluid)
     err, _ = field_errors(g, o)
     assert eN < 1e-13 and eB < 1e-13 and max(err.values()) < 1e-11, (eN, eB, err)
+    # without B planes (keep_B never called) B is still taken in: phi and the ghost values follow it
+    g2, o2 = make_pair(w, schedule=schedule)
+    g2.init(w.phi0); o2.init(w.phi0)
+    g2.set_populations(N2, B2); o2.set_populations(N2, B2)
+    g2.step(2); o2.step(2)
+    err2, _ = field_errors(g2, o2)
+    assert max(err2.values()) < 1e-11, err2
     # restart: N only (phi and the ghost values of the receiving context stay as they are)
     g.set_populations(N=N2)
     assert np.abs(g.get_populations(want_B=False)[0] - N2)[:, fluid].max() <= 1e-15
@@ -673,13 +712,17 @@ def test_paper_particle_at_interface_eq13():
 
 def test_layout_copy_helper_leaves_the_state_alone():
     w = wl.config5(seed=2, n=256)
-    g, _ = make_pair(w)
+    g, _ = make_pair(w, schedule=PAIR)                  # the helper measures the dense SoA layout (PAIR's)
     g.init(w.phi0); g.step(7)
     a = g.get()
     ms_copy = g.layout_copy_timed(3)
     g.step(5)
-    h, _ = make_pair(w)
+    h, _ = make_pair(w, schedule=PAIR)
     h.init(w.phi0); h.step(12)
+    p, _ = make_pair(w)                                 # compacted layouts keep no dense planes: refused, state untouched
+    p.init(w.phi0)
+    with pytest.raises(Exception):
+        p.layout_copy_timed(1)
     b, c = g.get(), h.get()
     assert ms_copy > 0
     for k in a:
