@@ -256,7 +256,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist, steps=None
         try:
             t_copy = sim.layout_copy_timed(20) * 1e-3
         except Exception:
-            t_copy = None
+            t_copy = None          # compacted layouts keep no dense planes: measured on a PAIR context below
         # ---- e2e through the C ABI with host buffers ----
         barrier()
         t0 = time.perf_counter()
@@ -302,6 +302,21 @@ def bench_precision(args, w, precision, schedule, device_index, dist, steps=None
     sim.close()
     del sim
     torch.cuda.empty_cache()
+    if t_copy is None and not light:
+        try:   # the dense SoA layout's plain-copy time, on a context that has that layout
+            aux = binding.LBM(binding.LBMParams(precision=precision, schedule=binding.SCHEDULE_PAIR, **w.param_dict()), w.mask, w.disks)
+            aux.init(phi0_h.numpy())
+            t_copy = aux.layout_copy_timed(20) * 1e-3
+            aux.close()
+            del aux
+            torch.cuda.empty_cache()
+            res["roofline"]["layout_copy"] = {
+                "what": "plain copy of every 32-byte sector of the 9 DENSE N planes and phi that holds a fluid node "
+                        "(lbm_layout_copy_timed on a PAIR context): what a pure streaming pass over the dense SoA-with-holes layout costs; "
+                        "the timed kernel runs on the compacted planes",
+                "ms": t_copy * 1e3, "frac": bytes_layout / t_copy / 1e9 / peak, "kernel_over_copy": t_collide / t_copy}
+        except Exception:
+            pass
     return res
 
 

@@ -29,8 +29,10 @@
  * Memory and ownership: every pointer is the caller's.  Pointers marked HOST must be host
  * memory (pageable or pinned) and are only used during the call; they are never retained.
  * `d_workspace` (DEVICE) is the only device memory a context uses — state, lists and the temporaries of
- * lbm_create alike (lbm_plan and the hook lbm_node_update_batch, which have no workspace, allocate and
- * free their own); it must stay allocated until lbm_destroy and be at least `workspace_bytes` (from lbm_plan) long, 256-byte
+ * lbm_create alike.  Three calls allocate and free their own: lbm_plan and the hook lbm_node_update_batch
+ * (they have no workspace), and lbm_keep_B(ctx, 1) under the compacted layouts (PACK, SPARSE), whose
+ * workspace holds no B planes (9 planes of nx*ny values, released by lbm_destroy).  The workspace must
+ * stay allocated until lbm_destroy and be at least `workspace_bytes` (from lbm_plan) long, 256-byte
  * aligned.  `cuda_stream` is a borrowed cudaStream_t (0 = default stream); all work of a context
  * is enqueued on it.  A context is not thread-safe; different contexts are independent.
  *
@@ -68,9 +70,9 @@ enum {
                                  (FFMA2).  Needs even nx, else FUSED is used                        */
   LBM_SCHEDULE_PACK = 5,      /* the PAIR kernel on pair-compacted population planes: a plane stores
                                  only the node pairs that hold a fluid node, row after row, without
-                                 holes (addressed through a 1-bit-per-pair mask + prefix table).  The
-                                 dense planes are kept as a mirror that lbm_get / lbm_diag / ... refresh
-                                 on demand.  Needs even nx, else FUSED is used                      */
+                                 holes (addressed through a 1-bit-per-pair mask + prefix table).  No
+                                 dense copy exists: lbm_get / lbm_diag / ... read the compact planes.
+                                 Needs even nx, else FUSED is used                                  */
   LBM_SCHEDULE_SPARSE = 6     /* the PACK layout with lanes mapped to fluid groups: one persistent CTA
                                  per SM, rows brought on chip by 1-D bulk copies (TMA) into a shared-memory
                                  ring, consumer warps work on 32 consecutive entries of the active-group
@@ -153,9 +155,11 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B);
  * the oracle does after its set_populations.  Synchronises. */
 int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B);
 
-/* Every schedule but BASELINE: when on != 0 the last time step of every lbm_step call also
- * writes the post-collision B_i* to HBM (workspace is sized for it) so that lbm_get_populations can return
- * B_i.  No effect on the arithmetic.  Ignored by the BASELINE schedule (B always stored). */
+/* Every schedule but BASELINE: when on != 0 the last time step of every lbm_step call also writes the
+ * post-collision B_i* to HBM so that lbm_get_populations / lbm_sample_populations can return B_i; set before
+ * lbm_init it keeps the initial B_i too.  No effect on the arithmetic.  Dense layouts (FUSED, PAIR) have the
+ * planes in their workspace; the compacted layouts (PACK, SPARSE, hence AUTO) allocate them with cudaMalloc on the
+ * first call with on != 0 (LBM_ECUDA if that fails).  Ignored by the BASELINE schedule (B always stored). */
 int lbm_keep_B(lbm_ctx* ctx, int32_t on);
 
 /* Populations at selected nodes only (for parity checks at sizes where 18 full arrays are too

@@ -29,7 +29,8 @@ int lbm_step_timed(lbm_ctx* ctx, int64_t n, double ms[3]);
  * a fluid node is read and written once; no halos, no arithmetic; destination is scratch memory, the
  * state is not disturbed) and returns the mean device time of one pass in milliseconds.  bench.py
  * reports it beside the roofline fraction: it is what a pure streaming pass over this layout costs.
- * LBM_EINVAL if nx*ny is not a whole number of sectors. */
+ * LBM_EINVAL if nx*ny is not a whole number of sectors, and for contexts of the compacted layouts (PACK, SPARSE,
+ * AUTO), which keep no dense planes: create the context with LBM_SCHEDULE_PAIR to measure. */
 int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass);
 
 /* Device-timing helper: per-kernel-kind accumulated launch counts since the last reset;
