@@ -515,6 +515,8 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   // rows per warp march: long marches amortise the halo rows; small grids need enough CTAs
   int TY = LBM_PAIR_TY;
   while (TY > 8 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 8) TY >>= 1;
+  // very small grids (less than two CTAs per SM even then): the march itself is what a launch-bound step waits for
+  while (TY > 2 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 2) TY >>= 1;
   const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
   const size_t smem = sizeof(PairRing<V, DP, PACKED>) * WARPS;
   auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true, PACKED> : k_fused_pair<V, DP, WARPS, MINB, false, PACKED>;
