@@ -63,3 +63,14 @@ def test_no_cpu_fallback_without_device():
         pytest.skip("a CUDA device is present")
     with pytest.raises(binding.LBMError):
         binding.LBM(binding.LBMParams(nx=8, ny=8), np.zeros((8, 8), np.uint8))
+
+
+def test_workspace_bytes_is_host_only_and_monotone():
+    """lbm_workspace_bytes: pure host arithmetic (no device here), 0 on bad parameters, grows with the ghost bound."""
+    good = binding.LBMParams(nx=64, ny=48, precision=64)
+    a = binding.workspace_bytes(good, 0)
+    b = binding.workspace_bytes(good, 1000)
+    assert 0 < a < b
+    assert binding.workspace_bytes(binding.LBMParams(nx=64, ny=48, precision=32), 1000) < b
+    assert binding.workspace_bytes(binding.LBMParams(nx=2, ny=48), 10) == 0          # nx < 3
+    assert binding.workspace_bytes(binding.LBMParams(nx=64, ny=48, W=3.0), 10) == 0   # W < 4 (PAPER.md:80)

@@ -246,6 +246,18 @@ def test_config1_1000_steps_fp64(schedule):
     assert abs(g.diag()["sum_phi"] - m0) < 1e-10 * m0
 
 
+def test_workspace_bytes_bounds_the_plan():
+    """The host-only upper bound is never below what lbm_plan computes from the mask, for every layout."""
+    from paper_2605_30878_b200 import binding
+    for w in (wl.config1(seed=0), wl.config5(seed=1, n=256), wl.config4(seed=0, nx=256, ny=64)):
+        for prec in (64, 32):
+            for sched in (0, BASELINE, FUSED, PAIR, PACK, SPARSE):
+                prm = binding.LBMParams(precision=prec, schedule=sched, **w.param_dict())
+                s = binding.LBM(prm, w.mask, w.disks)
+                assert binding.workspace_bytes(prm, s.n_ghost) >= s.workspace_bytes, (w.name, prec, sched)
+                s.close()
+
+
 def test_config1_1000_steps_through_cuda_graphs():
     """Small grids are launch-bound: off the legacy default stream lbm_step replays CUDA graphs
     of 32 steps.  Same 1,000-step parity run as above, same bar, and the launch bookkeeping still counts every
