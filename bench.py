@@ -180,14 +180,19 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def csrc_digest() -> str:
-    """sha1 of the kernel sources: a recorded ncu capture is only quoted for the build it was taken from."""
+def csrc_digest(root: str = None) -> str:
+    """sha1 of the kernel sources with comments and whitespace removed: a recorded ncu capture is only quoted for
+    the code it was taken from (editing a comment does not change the code)."""
     import hashlib
+    import re
     h = hashlib.sha1()
-    d = os.path.join(ROOT, "paper_2605_30878_b200", "csrc")
+    d = os.path.join(root or ROOT, "paper_2605_30878_b200", "csrc")
     for f in sorted(os.listdir(d)):
         if f.endswith((".cu", ".cuh")):
-            h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+            src = open(os.path.join(d, f), encoding="utf-8").read()
+            src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+            src = re.sub(r"//[^\n]*", "", src)
+            h.update(f.encode()); h.update("".join(src.split()).encode())
     return h.hexdigest()[:12]
 
 

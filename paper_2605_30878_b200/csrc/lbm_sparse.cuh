@@ -1,27 +1,32 @@
 // lbm_sparse.cuh — SPARSE schedule: the fused pull-stream + collide + segregation + phi(t+1) kernel with
 // lanes mapped to FLUID GROUPS instead of columns.
 //
-// State: the group-compacted planes of the PACK schedule (lbm_kernels.cuh: k_pair_mask, ptab) — a plane
-// stores only the aligned groups of NL x-adjacent nodes that hold a fluid node, row after row.  What
-// changes is who works on what:
+// State: group-compacted planes as under PACK (lbm_kernels.cuh: k_pair_mask, ptab) — only the aligned groups of NL
+// x-adjacent nodes that hold a fluid node are stored, row after row — but group-major: the nine 16-byte vectors of
+// a group are contiguous, so a row of a strip is ONE contiguous run.  What changes is who works on what:
 //
-//   * one persistent CTA per SM owns "marches": a strip of SP_S groups, a run of rows.  A row of a strip is
-//     a CONTIGUOUS run of the compact planes, so one producer warp brings every row on chip with eleven
-//     1-D bulk copies (cp.async.bulk -> UBLKCP, complete_tx on an mbarrier): nine population planes, the
-//     per-group metadata, the dense phi row.  Rows live in a shared-memory ring sized in entries, not rows.
-//   * the SP_W consumer warps take "passes": 32 consecutive ENTRIES of the row-major sequence of the
-//     strip's active groups (a pass may span several rows; 30 outputs + one helper lane per side).  Every
-//     lane therefore holds a group with a fluid node: no issue slot is spent on solid lanes.
+//   * one persistent CTA per SM owns "marches": a strip of at most SP_S groups, a run of rows (lbm_create cuts the
+//     work into marches of equal weight: one wave, no tail).
+//   * SP_K loader warps (rows split by parity) bring every row on chip with three 1-D bulk copies (cp.async.bulk
+//     -> UBLKCP, complete_tx on the row slot's mbarrier): the row's run of the compact planes, its group metadata,
+//     its dense phi row.  Rows live in a shared-memory ring sized in entries, not rows.
+//   * the SP_W consumer warps take "passes" from an atomic counter: 32 consecutive ENTRIES of the row-major
+//     sequence of the strip's active groups (a pass may span several rows; 30 outputs + one helper lane per
+//     side).  Every lane therefore holds a group with a fluid node: no issue slot is spent on solid lanes.
 //   * propagation (A16-A17) is a gather from the ring: same-row neighbours are the adjacent entries, the
 //     groups above / below are found by popcount on the row's group mask.  Half-way bounce-back (R12)
 //     selects the node's own opposite population, as in the PAIR kernel.
-//   * phi(x, t+1) = sum_q B_q*(x - c_q, t) (A13): every output lane writes the three partial sums its row
-//     sends to the rows above / at / below (x-moves by warp shuffle between x-adjacent lanes) into dense
-//     per-row buffers, each address written by exactly one lane; the producer warp adds the three rows
-//     once all consumers are past them and stores phi(t+1).  No atomics: results are run-to-run identical.
-//   * synchronisation: one mbarrier per row slot (producer -> consumers, TMA transaction bytes), one
-//     monotone "last row I am done with" counter per consumer warp (consumers -> producer) and one
-//     monotone counter for the partial-sum buffers.  No __syncthreads inside a march.
+//   * phi(x, t+1) = sum_q B_q*(x - c_q, t) (A13): every output lane writes the three partial sums its row sends to
+//     the rows above / at / below (x-moves by warp shuffle between x-adjacent lanes, direct stores into the columns
+//     of a neighbour group without a lane) into per-entry slots of the TARGET row, each address written by exactly
+//     one lane; SP_K finaliser warps add the three once all consumers are past the row and store phi(t+1).  No
+//     atomics on data: results are run-to-run identical.
+//   * synchronisation: one mbarrier per row slot (loader -> consumers, TMA transaction bytes), one monotone "no
+//     claim on the rows below R" counter per consumer warp (consumers -> finalisers) and one monotone "retired"
+//     counter per row class (finaliser -> loader).  No __syncthreads inside a march; every wait is bounded (a
+//     schedule bug traps after ~4 s instead of hanging the device).
+//   Measured (profiles/r2_sparse.txt): correct, but slower than PACK — the gather costs the instructions the fuller
+//   lanes save, and the ring leaves under two rows of look-ahead in 227 KB.  PACK stays the AUTO schedule.
 #pragma once
 #include "lbm_pair.cuh"
 
@@ -34,7 +39,7 @@ namespace lbm {
 #define LBM_SP_CAP 928
 #endif
 constexpr int SP_S = 126;                 // body groups of a strip; S + 2 halo groups = 128 mask bits
-constexpr int SP_W = LBM_SP_WARPS;        // consumer warps (+ 1 producer warp)
+constexpr int SP_W = LBM_SP_WARPS;        // consumer warps
 constexpr int SP_NR = 16;                 // row slots (phi rows, row info, full barriers)
 constexpr int SP_CAP = LBM_SP_CAP;        // entries of the population ring
 constexpr int SP_TYMAX = 512;             // rows of a march
