@@ -257,6 +257,46 @@ def flat_interface(nx: int, ny: int, W: float = 4.0):
     return np.zeros((ny, nx), np.uint8), np.zeros((0, 3)), np.repeat(prof[:, None], nx, axis=1)
 
 
+# ---- the paper's own drop-on-a-cylinder set-up (§III.B, :128-134) ------------------------------
+def _lens_area(R: float, Rc: float, d: float) -> float:
+    """Area common to two circles of radii R, Rc whose centres are d apart (textbook formula)."""
+    if d >= R + Rc:
+        return 0.0
+    if d <= abs(R - Rc):
+        return math.pi * min(R, Rc) ** 2
+    a = R * R * math.acos((d * d + R * R - Rc * Rc) / (2.0 * d * R))
+    b = Rc * Rc * math.acos((d * d + Rc * Rc - R * R) / (2.0 * d * Rc))
+    c = 0.5 * math.sqrt((-d + R + Rc) * (d + R - Rc) * (d - R + Rc) * (d + R + Rc))
+    return a + b - c
+
+
+def drop_on_cylinder_paper(theta_deg: float = 30.0, R: float = 40.0, A: float = 3000.0, W: float = 4.0,
+                           rho_ratio: float = 1000.0, mu_ratio: float = 100.0, sigma: float = 1e-2,
+                           x_offset: float = 0.0) -> Workload:
+    """(5R, 5R) periodic box, cylinder of radius R at (Lx/2, Ly/4), liquid of area A initialised as the circular
+    cap that meets the cylinder at the prescribed angle ("we initialize the drop with the expected equilibrium
+    configuration", PAPER.md:132): R_c from {pi R_c^2 - lens(R, R_c, d) = A, d^2 = R^2 + R_c^2 - 2 R R_c cos(theta)}."""
+    n = int(round(5.0 * R))
+    ct = math.cos(math.radians(theta_deg))
+    lo, hi = 1e-6, 100.0 * math.sqrt(A)
+    for _ in range(200):                       # bisection on R_c: the liquid area grows with it
+        Rc = 0.5 * (lo + hi)
+        d = math.sqrt(R * R + Rc * Rc - 2.0 * R * Rc * ct)
+        if math.pi * Rc * Rc - _lens_area(R, Rc, d) < A:
+            lo = Rc
+        else:
+            hi = Rc
+    cx, cy = 0.5 * n + x_offset, 0.25 * n
+    disks = np.array([[cx, cy, R]])
+    phi0 = drop_profile(n, n, cx, cy + d, Rc, W)
+    nu_l, nu_g = viscosities(rho_ratio, mu_ratio)
+    w = Workload(f"drop_on_cylinder_paper_{n}_theta{theta_deg:g}", n, n, rasterize_disks(n, n, disks), disks, phi0,
+                 rho_l=rho_ratio * RHO_G, rho_g=RHO_G, nu_l=nu_l, nu_g=nu_g, sigma=sigma, W=W,
+                 theta_deg=theta_deg, steps=20000, seed=0)
+    w.meta.update(Rc=Rc, d=d, hmax=d + Rc, area=A, R=R)
+    return w
+
+
 # ---- NEXT row f3: drop on a flat plate (§III.A, :102-124) -----------------------------------
 def flat_plate(theta_deg: float = 60.0, W: float = 4.0, scale: float = 1.0, rho_ratio: float = 1000.0,
                mu_ratio: float = 100.0, sigma: float = 1e-2, x_offset: float = 0.0) -> Workload:
