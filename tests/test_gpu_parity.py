@@ -246,6 +246,46 @@ def test_config1_1000_steps_fp64(schedule):
     assert abs(g.diag()["sum_phi"] - m0) < 1e-10 * m0
 
 
+@pytest.mark.parametrize("schedule", [pytest.param(0, id="auto"), pytest.param(SPARSE, id="sparse"), pytest.param(FUSED, id="fused")])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_mirror_and_rotation_equivariance(schedule, precision):
+    """Symmetry tests that need no oracle: mirroring the whole set-up about a vertical line mirrors the
+    result, rotating it by 90 degrees rotates it (u as a vector).  The kernels treat x (lanes, strips, shuffles) and
+    y (marches, ring slots) very differently, so a rotated run exercises the other code path on the same physics.
+    Sizes are ragged (several strips, a tail) and the drop is off every symmetry axis (R16)."""
+    from paper_2605_30878_b200 import binding
+    ny, nx = 132, 188
+    disks = np.array([[70.3, 40.6, 21.0], [150.2, 95.4, 14.5]])
+    mask = wl.rasterize_disks(nx, ny, disks)
+    phi0 = wl.drop_profile(nx, ny, 81.7, 77.2, 24.0, 4.0)
+    prm = dict(rho_l=50.0, rho_g=1.0, nu_l=0.05, nu_g=0.1, sigma=0.01, W=4.0, theta_deg=65.0, mobility=0.02, gx=2e-7, gy=-1e-7)
+
+    def run(mask, disks, phi0, gx, gy):
+        p = dict(prm); p.update(gx=gx, gy=gy)
+        s = binding.LBM(binding.LBMParams(nx=mask.shape[1], ny=mask.shape[0], precision=precision, schedule=schedule, **p), mask, disks)
+        s.init(phi0); s.step(60)
+        out = s.get()
+        s.close()
+        return out
+
+    a = run(mask, disks, phi0, prm["gx"], prm["gy"])
+    tol = 1e-12 if precision == 64 else 2e-5
+    # mirror x -> nx - 1 - x
+    dm = disks.copy(); dm[:, 0] = (nx - 1) - dm[:, 0]
+    b = run(mask[:, ::-1].copy(), dm, phi0[:, ::-1].copy(), -prm["gx"], prm["gy"])
+    for k, sgn in (("phi", 1), ("rho", 1), ("p", 1), ("ux", -1), ("uy", 1)):
+        sc = prm["rho_l"] if k == "rho" else 1.0
+        assert np.abs(a[k] - sgn * b[k][:, ::-1]).max() <= tol * sc, ("mirror", k)
+    # rotation by 90 degrees: (x, y) -> (-y, x) on the lattice, i.e. array transpose + flip; u rotates with it
+    dr = np.stack([(ny - 1) - disks[:, 1], disks[:, 0], disks[:, 2]], axis=1)
+    c = run(np.ascontiguousarray(mask.T[:, ::-1]), dr, np.ascontiguousarray(phi0.T[:, ::-1]), -prm["gy"], prm["gx"])
+    back = lambda f: f[:, ::-1].T                       # noqa: E731  undo the rotation of the arrays
+    for k in ("phi", "rho", "p"):
+        sc = prm["rho_l"] if k == "rho" else 1.0
+        assert np.abs(a[k] - back(c[k])).max() <= tol * sc, ("rotation", k)
+    assert np.abs(a["ux"] - back(c["uy"])).max() <= tol and np.abs(a["uy"] + back(c["ux"])).max() <= tol
+
+
 def test_workspace_bytes_bounds_the_plan():
     """The host-only upper bound is never below what lbm_plan computes from the mask, for every layout."""
     from paper_2605_30878_b200 import binding
