@@ -13,9 +13,10 @@
  * conservation, Laplace law at density ratio 1 and 1000, contact angle on a cylinder, single-phase
  * and two-layer Poiseuille, rotational covariance of the node's force).  The correction forces
  * F_visc (A11, R10), F_p (A10) and the harmonic viscosity rule (R6) are pinned by
- * tests/test_oracle_forces.py.  Conventions that no independent fact fixes stay "parity unpinned":
- * R5 (reference pressure 0), R9 (one Picard pass rather than a converged iteration), R14 (initial
- * populations), R15 (plain bilinear interpolation whatever the corner's class).
+ * tests/test_oracle_forces.py, which also measures the mobility of the color equation (R5).
+ * Conventions that no independent fact fixes stay "parity unpinned": R9 (one Picard pass rather than
+ * a converged iteration), R14 (no anti-diffusion part in the initial B_i; the moments of the initial
+ * state are pinned), R15 (plain bilinear interpolation whatever the corner's class).
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared -o liblbmref.so lbmref.c -lm
  */

@@ -15,6 +15,8 @@ None of these re-types the oracle's formula.  What they check, and which mistake
   spin-2 tensor, grad phi as a vector) by 90 and by 45 degrees must rotate the returned force with
   them.  The 45-degree case mixes Pi_xx - Pi_yy with Pi_xy, so it fails if the factor 1/2 on m7 is
   dropped or the two gradients are exchanged in one component.
+* `test_mobility_of_the_color_equation`: the decay rate of a sine wave of phi with the anti-diffusion switched off is
+  M_phi: pins R5 (alpha = 1 - 10 M_phi / 3 at reference pressure 0) and, with it, the segregation + streaming of B.
 * `test_laplace_law_density_ratio_1000`: Delta p_h = rho_l p_in - rho_g p_out = sigma / R with
   p_h = rho p (:278): fails if F_p = -p grad rho is dropped or has the wrong sign (the pressure jump
   then sits on p, not on rho p).
@@ -127,3 +129,22 @@ def test_laplace_law_density_ratio_1000():
     # the jump is carried by rho p: p itself is three orders of magnitude smaller inside the liquid
     assert abs(g["p"][n // 2, n // 2]) < 5e-3 * sigma / Reff
     assert d["umax"] < 1e-4
+
+
+@pytest.mark.parametrize("mobility", [0.02, 0.05])
+def test_mobility_of_the_color_equation(mobility):
+    """R5: alpha is never printed, only M_phi = 0.02 and M_phi = c_s^2 dt/2 [9(1 - alpha)/5 + p/c_s^2]
+    (:288); the oracle takes the reference pressure p = 0, i.e. alpha = 1 - 10 M_phi / 3.  The pin measures the
+    mobility the scheme actually has: with the anti-diffusion switched off (W -> infinity; Eq. 3, :41) and the fluid at
+    rest, a small sine wave of phi must decay as exp(-M_phi k^2 t).  Any other reading of alpha shows up one to one
+    in the measured rate (recorded: 0.9991 M_phi, the rest is the O(k^2) lattice correction)."""
+    nx, ny, a0, T = 64, 4, 0.01, 4000
+    k = 2.0 * math.pi / nx
+    phi0 = 0.5 + a0 * np.sin(k * np.arange(nx))[None, :] * np.ones((ny, 1))
+    prm = ref.RefParams(nx=nx, ny=ny, rho_l=1.0, rho_g=1.0, nu_l=1 / 6, nu_g=1 / 6, sigma=0.0, W=1e7, mobility=mobility)
+    s = ref.RefLBM(prm, np.zeros((ny, nx), np.uint8)); s.init(phi0); s.step(T)
+    g = s.get()
+    row = g["phi"][0]
+    a = 2.0 * abs(np.fft.rfft(row - row.mean())[1]) / nx
+    assert -math.log(a / a0) / (k * k * T) == pytest.approx(mobility, rel=5e-3)
+    assert np.abs(g["phi"] - row[None, :]).max() < 1e-15 and max(np.abs(g["ux"]).max(), np.abs(g["uy"]).max()) < 1e-12

@@ -37,6 +37,35 @@ def test_uniform_phase_at_rest_is_a_fixed_point():
         assert np.abs(g["ux"]).max() < 1e-16 and np.abs(g["p"]).max() < 1e-14
 
 
+def test_initial_state_carries_the_prescribed_moments():
+    """R14 (the paper is silent on the initial populations): N_i = N_i^eq(p = 0, u0), B_i = phi0 N_i.  What the paper
+    does fix are the moments (A13-A15, :311-315): right after lbm_init phi = phi0, u = u0 and p = 0 where no force
+    acts, and a uniform stream is an exact fixed point (the initial N is the equilibrium, not something that relaxes
+    to it).  The anti-diffusion part of B_i is not in the initial state; the first collision puts it there."""
+    rng = np.random.default_rng(3)
+    n = 24
+    yy, xx = np.mgrid[0:n, 0:n]
+    phi0 = 0.5 + 0.3 * np.sin(2 * np.pi * xx / n) * np.cos(2 * np.pi * yy / n)
+    u0 = 1e-3 * rng.standard_normal((2, n, n))
+    prm = ref.RefParams(nx=n, ny=n, rho_l=1.0, rho_g=1.0, nu_l=1 / 6, nu_g=1 / 6, sigma=0.0, W=4.0)
+    s = ref.RefLBM(prm, np.zeros((n, n), np.uint8)); s.init(phi0, u0)
+    g = s.get()
+    N, B = s.get_populations()
+    assert np.abs(g["phi"] - phi0).max() < 1e-15 and np.abs(B.sum(axis=0) - phi0).max() < 1e-15
+    assert np.abs(g["ux"] - u0[0]).max() < 1e-15 and np.abs(g["uy"] - u0[1]).max() < 1e-15
+    assert np.abs(g["p"]).max() < 1e-15 and np.abs(N.sum(axis=0) - 1.0).max() < 1e-15
+    # uniform stream, uniform phase, density ratio 1000: nothing changes, to the last bit of u
+    uu = np.zeros((2, n, n)); uu[0] = 3e-3; uu[1] = -1e-3
+    prm = ref.RefParams(nx=n, ny=n, rho_l=1000.0, rho_g=1.0, nu_l=0.01, nu_g=0.1, sigma=0.01, W=4.0)
+    s = ref.RefLBM(prm, np.zeros((n, n), np.uint8)); s.init(np.ones((n, n)), uu)
+    N0, _ = s.get_populations()
+    s.step(50)
+    N1, _ = s.get_populations()
+    g = s.get()
+    assert np.abs(N1 - N0).max() < 1e-15
+    assert np.abs(g["ux"] - 3e-3).max() < 1e-15 and np.abs(g["uy"] + 1e-3).max() < 1e-15
+
+
 def test_mass_of_each_phase_is_conserved_with_solids_and_walls():
     """PAPER.md:156 "respective amounts of liquid and gas in the system are conserved"; bounce-back
     returns what leaves, segregation has sum B* = phi."""
