@@ -181,14 +181,15 @@ def run_reference(args):
 
 
 def csrc_digest(root: str = None) -> str:
-    """sha1 of the kernel sources with comments and whitespace removed: a recorded ncu capture is only quoted for
-    the code it was taken from (editing a comment does not change the code)."""
+    """sha1 of the kernel sources (csrc/*.cuh: kernels and their launchers) with comments and whitespace removed: a
+    recorded ncu capture is only quoted for the kernel code it was taken from (editing a comment, or the host-side
+    API file, does not change the kernels)."""
     import hashlib
     import re
     h = hashlib.sha1()
     d = os.path.join(root or ROOT, "paper_2605_30878_b200", "csrc")
     for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
+        if f.endswith(".cuh"):
             src = open(os.path.join(d, f), encoding="utf-8").read()
             src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
             src = re.sub(r"//[^\n]*", "", src)

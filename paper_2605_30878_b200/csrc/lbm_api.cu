@@ -470,7 +470,7 @@ PopView<R> B_view(const lbm_ctx* c) {
 
 extern "C" {
 
-const char* lbm_version(void) { return "liblbm_b200 0.1 (sm_100a)"; }
+const char* lbm_version(void) { return "liblbm_b200 0.2 (sm_100a)"; }
 
 const char* lbm_last_error(const lbm_ctx* ctx) { return ctx ? ctx->err : g_err; }
 
