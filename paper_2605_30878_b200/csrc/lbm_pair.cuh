@@ -512,11 +512,27 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   constexpr int OUTC = 30 * LaneOf<V>::NL;
   const int nwx = (C.nx + OUTC - 1) / OUTC;
   const int gx = (nwx + WARPS - 1) / WARPS;
-  // rows per warp march: long marches amortise the halo rows; small grids need enough CTAs
+  // Rows per warp march.  Long marches amortise the two halo rows and the pipeline fill (about 5 rows' worth); short
+  // ones make more CTAs.  A launch takes about waves x (TY + 5) row times, waves = ceil(CTAs / resident CTAs of the
+  // device): take the TY that minimises it; marches longer than 16 rows only when they still fill the device once
+  // (a single under-filled wave of long marches lost to three waves of short ones: measured on 1024^2 ... 8192^2
+  // and the paper's 1500 x 900, profiles/r2_small_grids.md).
+  int nsm = 148;
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  }
+  const long long slots = (long long)nsm * MINB;
   int TY = LBM_PAIR_TY;
-  while (TY > 8 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 8) TY >>= 1;
+  long long best = -1;
+  for (int t = LBM_PAIR_TY; t >= 8; t >>= 1) {
+    const long long ctas = (long long)gx * ((C.ny + t - 1) / t);
+    if (t > 16 && ctas < slots) continue;
+    const long long cost = ((ctas + slots - 1) / slots) * (t + 5);
+    if (best < 0 || cost < best) { best = cost; TY = t; }
+  }
   // very small grids (less than two CTAs per SM even then): the march itself is what a launch-bound step waits for
-  while (TY > 2 && (long long)gx * ((C.ny + TY - 1) / TY) < 148 * 2) TY >>= 1;
+  while (TY > 2 && (long long)gx * ((C.ny + TY - 1) / TY) < nsm * 2) TY >>= 1;
   const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
   const size_t smem = sizeof(PairRing<V, DP, PACKED>) * WARPS;
   auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true, PACKED> : k_fused_pair<V, DP, WARPS, MINB, false, PACKED>;
