@@ -350,6 +350,8 @@ def main():
     ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "pair", "pack", "sparse"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the 2048^2 / 4096^2 points of config 5")
+    ap.add_argument("--plain-launches", action="store_true",
+                    help="run on the legacy default stream, where lbm_step cannot replay CUDA graphs (A/B for the small grids)")
     ap.add_argument("--reference-budget", type=float, default=120.0, help="seconds of CPU work the --impl reference arm may spend")
     ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r2_traffic.csv"),
                     help="ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel "
@@ -392,7 +394,7 @@ def main():
         workload = f"BASELINE config {args.config} ({w.name}) {w.nx}x{w.ny}"
     # all library work goes to a non-default stream (torch's current stream inside this block): the legacy default
     # stream cannot be captured, and lbm_step replays CUDA graphs on small grids; events are recorded on the same stream
-    side = torch.cuda.Stream()
+    side = torch.cuda.default_stream() if args.plain_launches else torch.cuda.Stream()
     with torch.cuda.stream(side):
         results = {p: bench_precision(args, w, p, sched, local, dist) for p in precs}
         sweep = {}
