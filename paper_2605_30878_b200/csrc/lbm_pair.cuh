@@ -53,17 +53,20 @@ inline bool ensure_smem_attr(const void* kern, size_t smem) {
 #ifndef LBM_PAIR_DP64
 #define LBM_PAIR_DP64 1
 #endif
+// One warp per CTA: the warps share nothing, and a CTA's slot (registers, ring) is only handed on when its last warp
+// has finished its march, so with 3-warp CTAs the warps that met more solid rows left their slots idle (11.2 of 12
+// warps resident on average at 8192^2; mid-size grids lost more: profiles/r2_small_grids.md).  MINB = warps per SM.
 #ifndef LBM_PAIR_MINB32
-#define LBM_PAIR_MINB32 5
+#define LBM_PAIR_MINB32 15
 #endif
 #ifndef LBM_PAIR_MINB64
-#define LBM_PAIR_MINB64 4
+#define LBM_PAIR_MINB64 12
 #endif
 #ifndef LBM_PAIR_MINBQ
-#define LBM_PAIR_MINBQ 4
+#define LBM_PAIR_MINBQ 12
 #endif
 #ifndef LBM_PAIR_WARPS
-#define LBM_PAIR_WARPS 3
+#define LBM_PAIR_WARPS 1
 #endif
 #ifndef LBM_PAIR_FULLSECTOR
 #define LBM_PAIR_FULLSECTOR 1
@@ -531,8 +534,8 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
     const long long cost = ((ctas + slots - 1) / slots) * (t + 5);
     if (best < 0 || cost < best) { best = cost; TY = t; }
   }
-  // very small grids (less than two CTAs per SM even then): the march itself is what a launch-bound step waits for
-  while (TY > 2 && (long long)gx * ((C.ny + TY - 1) / TY) < nsm * 2) TY >>= 1;
+  // very small grids (less than four warps per SM even then): the march itself is what a launch-bound step waits for
+  while (TY > 2 && (long long)nwx * ((C.ny + TY - 1) / TY) < nsm * 4) TY >>= 1;
   const dim3 grid((unsigned)gx, (unsigned)((C.ny + TY - 1) / TY), 1);
   const size_t smem = sizeof(PairRing<V, DP, PACKED>) * WARPS;
   auto kern = Bdst ? k_fused_pair<V, DP, WARPS, MINB, true, PACKED> : k_fused_pair<V, DP, WARPS, MINB, false, PACKED>;
