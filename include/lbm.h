@@ -155,6 +155,19 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B);
  * the oracle does after its set_populations.  Synchronises. */
 int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B);
 
+/* Rows of the state as one device buffer: the hand-over between the slabs of a 1-D domain decomposition along y
+ * (the path shards into slabs that exchange the populations and phi rows next to each cut; the method
+ * itself is local, A16-A17 :318-322 move a population by one node per step).  The complete state of a context at time
+ * t is phi(x, t) (fluid and ghost values) and the populations N_i; lbm_rows_export copies the part that belongs to
+ * the grid rows j0 <= j < j0 + nrows (no wrap) into d_buf (DEVICE, >= lbm_rows_bytes bytes, caller-owned),
+ * lbm_rows_import overwrites those rows from such a buffer.  The buffer is in the context's own storage format: it
+ * can only be imported by a context with the same nx, precision and schedule whose solid mask agrees on these rows
+ * (else LBM_EINVAL: the sizes differ).  Asynchronous on the context's stream; lbm_rows_bytes may synchronise once.
+ * Ghost-node geometry is not transferred: each context computes its own at lbm_create. */
+int lbm_rows_bytes(lbm_ctx* ctx, int32_t j0, int32_t nrows, size_t* bytes);
+int lbm_rows_export(lbm_ctx* ctx, int32_t j0, int32_t nrows, void* d_buf, size_t capacity);
+int lbm_rows_import(lbm_ctx* ctx, int32_t j0, int32_t nrows, const void* d_buf, size_t bytes);
+
 /* Every schedule but BASELINE: when on != 0 the last time step of every lbm_step call also writes the
  * post-collision B_i* to HBM so that lbm_get_populations / lbm_sample_populations can return B_i; set before
  * lbm_init it keeps the initial B_i too.  No effect on the arithmetic.  Dense layouts (FUSED, PAIR) have the

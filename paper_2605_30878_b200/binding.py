@@ -24,7 +24,8 @@ FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
 # include/lbm.h (the product boundary) and include/lbm_test.h (test and measurement hooks)
 EXPORTS = ("lbm_plan", "lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
-           "lbm_get_populations", "lbm_set_populations", "lbm_keep_B", "lbm_sample_populations",
+           "lbm_get_populations", "lbm_set_populations", "lbm_rows_bytes", "lbm_rows_export", "lbm_rows_import",
+           "lbm_keep_B", "lbm_sample_populations",
            "lbm_get_classification", "lbm_diag", "lbm_last_error", "lbm_version", "lbm_destroy")
 TEST_EXPORTS = ("lbm_node_update_batch", "lbm_step_timed", "lbm_layout_copy_timed", "lbm_launch_counts")
 
@@ -105,6 +106,9 @@ def load_library() -> C.CDLL:
         L.lbm_workspace_bytes.argtypes = [C.POINTER(_Params), i64]
         L.lbm_workspace_bytes.restype = C.c_size_t
         L.lbm_set_populations.argtypes = [vp, vp, vp]
+        L.lbm_rows_bytes.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
+        L.lbm_rows_export.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
+        L.lbm_rows_import.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
         L.lbm_create.argtypes = [C.POINTER(vp), C.POINTER(_Params), vp, vp, C.c_int32, vp,
                                  C.c_size_t, vp]
         L.lbm_init.argtypes = [vp, vp, vp]
@@ -265,6 +269,20 @@ class LBM:
         Ba = _f64(B, 9 * self.n) if B is not None else None
         _check(load_library().lbm_set_populations(self._h, Na.ctypes.data if Na is not None else None,
                                                   Ba.ctypes.data if Ba is not None else None), self._h)
+
+    def rows_bytes(self, j0: int, nrows: int) -> int:
+        """Bytes of the state that belongs to the grid rows j0 <= j < j0 + nrows (no wrap)."""
+        b = C.c_size_t()
+        _check(load_library().lbm_rows_bytes(self._h, int(j0), int(nrows), C.byref(b)), self._h)
+        return int(b.value)
+
+    def rows_export(self, j0: int, nrows: int, buf_ptr: int, capacity: int):
+        """Copies those rows of the state (phi and the populations) into a DEVICE buffer; asynchronous on the stream."""
+        _check(load_library().lbm_rows_export(self._h, int(j0), int(nrows), int(buf_ptr), int(capacity)), self._h)
+
+    def rows_import(self, j0: int, nrows: int, buf_ptr: int, nbytes: int):
+        """Overwrites those rows of the state from a DEVICE buffer another context exported; asynchronous."""
+        _check(load_library().lbm_rows_import(self._h, int(j0), int(nrows), int(buf_ptr), int(nbytes)), self._h)
 
     def sample_populations(self, idx, want_B: bool = False):
         idx = np.ascontiguousarray(idx, dtype=np.int64).reshape(-1)

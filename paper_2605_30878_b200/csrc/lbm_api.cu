@@ -74,6 +74,8 @@ struct lbm_ctx {
   size_t cps;        // compact plane stride in pairs
   uint2* ptab;
   void* Nc[2];
+  long long nfp;        // groups stored in a compact plane
+  unsigned* row_base;   // host, ny + 1: compact index of the first group of every row (lbm_rows_*; fetched on first use)
   // SPARSE schedule: per (strip, row) descriptors, per-group metadata, the marches of every CTA
   int sparse;
   int sp_nstrips, sp_ncta, sp_nmarch, sp_sw;
@@ -466,6 +468,48 @@ PopView<R> B_view(const lbm_ctx* c) {
 }
 
 
+// lbm_rows_*: the pieces of the state that belong to rows [j0, j0 + nrows): phi (dense rows) and the nine population
+// planes (dense rows, or the rows' run of groups in the compact planes; BASELINE: the nine B planes too).  Each piece
+// is one contiguous device range.
+struct RowPiece { char* p; size_t bytes; };
+int row_pieces(lbm_ctx* ctx, int j0, int nrows, RowPiece (&pc)[19], int* npc) {
+  const lbm_params& P = ctx->P;
+  if (j0 < 0 || nrows < 1 || (long long)j0 + nrows > P.ny) return fail(ctx, LBM_EINVAL, "rows outside the grid (ranges do not wrap)");
+  const size_t rs = ctx->is32 ? 4 : 8;
+  int k = 0;
+  pc[k++] = RowPiece{(char*)ctx->phi[ctx->pcur] + (size_t)j0 * P.nx * rs, (size_t)nrows * P.nx * rs};
+  if (!ctx->packed) {
+    const size_t ps = plane_stride(&P);
+    for (int q = 0; q < 9; q++)
+      pc[k++] = RowPiece{(char*)ctx->N[ctx->cur] + ((size_t)q * ps + (size_t)j0 * P.nx) * rs, (size_t)nrows * P.nx * rs};
+    if (!ctx->fused)   // BASELINE: the B_i are part of the stored state
+      for (int q = 0; q < 9; q++)
+        pc[k++] = RowPiece{(char*)ctx->B[ctx->cur] + ((size_t)q * ps + (size_t)j0 * P.nx) * rs, (size_t)nrows * P.nx * rs};
+  } else {
+    if (!ctx->row_base) {
+      unsigned* rb = (unsigned*)malloc(((size_t)P.ny + 1) * sizeof(unsigned));
+      if (!rb) return fail(ctx, LBM_ENOMEM, "host allocation failed");
+      // .y of the first table word of every row
+      cudaError_t e = cudaMemcpy2DAsync(rb, sizeof(unsigned), (const char*)ctx->ptab + sizeof(unsigned), (size_t)ctx->nw * sizeof(uint2),
+                                        sizeof(unsigned), (size_t)P.ny, cudaMemcpyDeviceToHost, ctx->st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->st);
+      if (e != cudaSuccess) { free(rb); return cuda_fail(ctx, e, "row table"); }
+      rb[P.ny] = (unsigned)ctx->nfp;
+      ctx->row_base = rb;
+    }
+    const size_t G = (size_t)pack_group((int)rs, P.nx);
+    const size_t g0 = ctx->row_base[j0], g1 = ctx->row_base[j0 + nrows];
+    char* base = (char*)ctx->Nc[ctx->ccur];
+    if (g1 > g0) {
+      if (ctx->sparse) pc[k++] = RowPiece{base + g0 * 9 * G * rs, (g1 - g0) * 9 * G * rs};   // group-major
+      else
+        for (int q = 0; q < 9; q++) pc[k++] = RowPiece{base + ((size_t)q * ctx->cps + g0) * G * rs, (g1 - g0) * G * rs};
+    }
+  }
+  *npc = k;
+  return LBM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -685,6 +729,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
     if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "pair table"); }
     if ((long long)last[0] + last[1] != nfp) { delete c; return fail(nullptr, LBM_EINVAL, "internal: fluid group counts of host and device differ"); }
     c->packed = 1;
+    c->nfp = nfp;
   }
   if (use_sparse(prm)) {   // SPARSE schedule: per-group metadata, per (strip, row) descriptors, marches
     const int G = pack_group(c->is32 ? 4 : 8, prm->nx);
@@ -727,6 +772,7 @@ void lbm_destroy(lbm_ctx* ctx) {
   for (auto& g : ctx->gexec)
     if (g) cudaGraphExecDestroy(g);
   if (ctx->B_owned) cudaFree(ctx->B[0]);
+  free(ctx->row_base);
   delete ctx;
 }
 
@@ -929,6 +975,51 @@ int lbm_get_populations(lbm_ctx* ctx, double* N, double* B) {
       CK(cudaStreamSynchronize(ctx->st));
     }
   }
+  return LBM_OK;
+}
+
+int lbm_rows_bytes(lbm_ctx* ctx, int32_t j0, int32_t nrows, size_t* bytes) {
+  if (!ctx || !bytes) return fail(ctx, LBM_EINVAL, "null argument");
+  RowPiece pc[19];
+  int n = 0;
+  const int rc = row_pieces(ctx, j0, nrows, pc, &n);
+  if (rc != LBM_OK) return rc;
+  size_t b = 0;
+  for (int i = 0; i < n; i++) b += pc[i].bytes;
+  *bytes = b;
+  return LBM_OK;
+}
+
+int lbm_rows_export(lbm_ctx* ctx, int32_t j0, int32_t nrows, void* d_buf, size_t cap) {
+  if (!ctx || !d_buf) return fail(ctx, LBM_EINVAL, "null argument");
+  RowPiece pc[19];
+  int n = 0;
+  const int rc = row_pieces(ctx, j0, nrows, pc, &n);
+  if (rc != LBM_OK) return rc;
+  size_t off = 0;
+  for (int i = 0; i < n; i++) {
+    if (off + pc[i].bytes > cap) return fail(ctx, LBM_ENOMEM, "row buffer too small (lbm_rows_bytes)");
+    CK(cudaMemcpyAsync((char*)d_buf + off, pc[i].p, pc[i].bytes, cudaMemcpyDeviceToDevice, ctx->st));
+    off += pc[i].bytes;
+  }
+  return LBM_OK;
+}
+
+int lbm_rows_import(lbm_ctx* ctx, int32_t j0, int32_t nrows, const void* d_buf, size_t bytes) {
+  if (!ctx || !d_buf) return fail(ctx, LBM_EINVAL, "null argument");
+  RowPiece pc[19];
+  int n = 0;
+  const int rc = row_pieces(ctx, j0, nrows, pc, &n);
+  if (rc != LBM_OK) return rc;
+  size_t need = 0;
+  for (int i = 0; i < n; i++) need += pc[i].bytes;
+  if (bytes != need) return fail(ctx, LBM_EINVAL, "row buffer size differs from lbm_rows_bytes: the two contexts do not agree on these rows");
+  size_t off = 0;
+  for (int i = 0; i < n; i++) {
+    CK(cudaMemcpyAsync(pc[i].p, (const char*)d_buf + off, pc[i].bytes, cudaMemcpyDeviceToDevice, ctx->st));
+    off += pc[i].bytes;
+  }
+  if (ctx->fused) ctx->B_valid = 0;   // B planes kept by lbm_keep_B no longer belong to this state
   return LBM_OK;
 }
 
