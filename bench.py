@@ -4,6 +4,7 @@ on BASELINE.json's config 5 (porous medium, density ratio 1000, theta = 110 deg)
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--reps R] [--impl ours|reference] [--config 1..5]
                     [--n 8192] [--precision 64|32|both] [--schedule auto|baseline|fused|pair|pack|sparse]
+                    [--slab [--exchange-every 4]] [--plain-launches] [--no-sweep] [--no-cpu-baseline]
 
 Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement"):
   value        MLUPS (Eq. 14: all grid nodes x steps / time / 1e6), device-resident state,
@@ -16,7 +17,8 @@ Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement"):
   reps         the K-step region is timed R times; ms_per_step and value are the median, best is reported too
   sweep        BASELINE config 5 names 2048^2, 4096^2, 8192^2: the two smaller sizes as extra keys
   cpu_baseline the CPU oracle timed on this box's host cores on a bounded sample (N = 1, rank 0 only)
-Multi-GPU: the path does not shard in this build ("replicas only"): N independent replicas.
+Multi-GPU: N independent replicas by default (north_star: one GPU, no sharding).  `--slab` runs ONE
+grid cut into N slabs along y with a halo exchange every `--exchange-every` steps instead (strong scaling).
 """
 from __future__ import annotations
 
@@ -326,6 +328,102 @@ def bench_precision(args, w, precision, schedule, device_index, dist, steps=None
     return res
 
 
+def bench_slab(args, w, precision, schedule, device_index, dist, rank, world, workload):
+    """`--slab`: ONE grid cut into `world` slabs along y (paper_2605_30878_b200/slab.py): strong scaling.
+    Every rank runs its rows plus the halos; every `--exchange-every` steps the halo rows are exchanged with the two
+    neighbours (NCCL send/recv; with one rank: the slab's own other end).  Same timing rules as the replica mode."""
+    import torch
+    from paper_2605_30878_b200 import binding, slab
+    prm = binding.LBMParams(precision=precision, schedule=schedule, **w.param_dict())
+    rs = 8 if precision == 64 else 4
+    t0 = time.perf_counter()
+    sl = slab.Slab(prm, w.mask, w.disks, rank, world, steps_per_exchange=args.exchange_every)
+    t_create = time.perf_counter() - t0
+    sl.init(w.phi0)
+    slab.run(sl, args.warmup, dist)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(device_index)
+    sl.sim.launch_counts(reset=True)
+    barrier()
+    sampler.start()
+    rep_ms = []
+    for _ in range(args.reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        slab.run(sl, args.steps, dist)
+        e1.record()
+        barrier()
+        rep_ms.append(e0.elapsed_time(e1))
+    clocks = sampler.stop()
+    launches = sl.sim.launch_counts()
+    n_launch = (launches["collide"] + launches["phi_sum"] + launches["ghost"]) // args.reps
+    rep_ms = [max_over_ranks([m], dist, "cuda")[0] for m in rep_ms]
+    ms = float(np.median(rep_ms))
+    # the exchange alone (pack, send/recv, unpack), and the local kernels alone
+    n_ex = 20
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n_ex):
+        slab.exchange_distributed(sl, dist)
+    e1.record()
+    barrier()
+    ms_exchange = max_over_ranks([e0.elapsed_time(e1) / n_ex], dist, "cuda")[0]
+    split = sl.sim.step_timed(min(args.steps, 200))
+    ks = min(args.steps, 200)
+    t_collide = split["collide"] / ks * 1e-3
+    # end to end: host phi0 of the whole grid -> slabs -> steps -> owned rows back on the host
+    barrier()
+    t0 = time.perf_counter()
+    sl.init(w.phi0)
+    slab.run(sl, args.steps, dist)
+    own = sl.get()
+    torch.cuda.synchronize()
+    t_e2e = max_over_ranks([time.perf_counter() - t0], dist, "cuda")[0]
+
+    n = w.nx * w.ny
+    rows = np.arange(sl.y0 - sl.H, sl.y1 + sl.H) % w.ny
+    nf_local = int((np.asarray(w.mask).reshape(w.ny, w.nx)[rows] == 0).sum())
+    nf_owned = int((np.asarray(w.mask).reshape(w.ny, w.nx)[sl.y0:sl.y1] == 0).sum())
+    bytes_layout = nf_local * 20 * rs + 2 * sl.nl * w.nx
+    peak, peak_src = measured_peak()
+    ex_bytes = sum(sl._nb.values())
+    res = {
+        "metric": METRIC, "value": n * args.steps / (ms * 1e-3) / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f64" if precision == 64 else "f32", "data": "synthetic",
+        "config": {"workload": workload, "parallelism": f"slab{world}: one grid cut into {world} slab(s) along y",
+                   "rows_owned": sl.n_own, "halo_rows": sl.H, "geometry_margin_rows": sl.margin,
+                   "steps_per_exchange": sl.k, "exchange_bytes_sent_per_rank": ex_bytes // 2,
+                   "redundant_rows_frac": 2.0 * sl.H / sl.n_own, "schedule": args.schedule,
+                   "n_fluid_owned": nf_owned, "create_s": t_create,
+                   "l2": "state of a slab >> 126 MB L2 (inputs larger than L2, no flush needed)"},
+        "reps": {"n": args.reps, "ms_per_step": [m / args.steps for m in rep_ms], "best_ms_per_step": min(rep_ms) / args.steps},
+        "e2e": {"value": n * args.steps / t_e2e / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": sl.nl * w.nx * 8 / args.steps,
+                "d2h_bytes_per_step": 5 * sl.n_own * w.nx * 8 / args.steps,
+                "what": "Slab.init(host phi0) + slab.run(K) + Slab.get(5 host fields of the owned rows), wall clock"},
+        "gpu_launches": n_launch, "clocks": clocks,
+        "exchange_ms": ms_exchange, "exchange_ms_per_step": ms_exchange / sl.k,
+        "kernel_ms_per_step": {k: v / ks for k, v in split.items()},
+        "roofline": {"bound": "hbm", "achieved": bytes_layout / t_collide / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": bytes_layout / t_collide / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "kernel": "k_fused_pair", "kernel_ms": t_collide * 1e3, "bytes_per_launch": bytes_layout,
+                     "note": "the rank's local grid (owned rows + 2 H halo rows); bytes as in the replica mode"},
+        "cpu_baseline": None,
+        "check": {"phi_min": float(own["phi"].min()), "phi_max": float(own["phi"].max()),
+                  "finite": bool(np.isfinite(own["phi"]).all() and np.isfinite(own["ux"]).all())},
+    }
+    sl.close()
+    return res
+
+
 SMALL_CONFIGS = {
     # BASELINE.json configs 1-4: parity-test cases first; their MLUPS are reported beside the paper's Table I rows as
     # context (PAPER.md:237: small grids under-utilise the GPU).  (workload, precisions, timed steps)
@@ -352,6 +450,9 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the 2048^2 / 4096^2 points of config 5")
     ap.add_argument("--plain-launches", action="store_true",
                     help="run on the legacy default stream, where lbm_step cannot replay CUDA graphs (A/B for the small grids)")
+    ap.add_argument("--slab", action="store_true",
+                    help="N > 1 (or 1): ONE grid cut into N slabs along y with a halo exchange, instead of N replicas (strong scaling)")
+    ap.add_argument("--exchange-every", type=int, default=4, help="--slab: time steps between two halo exchanges")
     ap.add_argument("--reference-budget", type=float, default=120.0, help="seconds of CPU work the --impl reference arm may spend")
     ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r2_traffic.csv"),
                     help="ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel "
@@ -382,7 +483,7 @@ def main():
     sched = {"auto": binding.SCHEDULE_AUTO, "baseline": binding.SCHEDULE_BASELINE, "fused": binding.SCHEDULE_FUSED,
              "pair": binding.SCHEDULE_PAIR, "pack": binding.SCHEDULE_PACK, "sparse": binding.SCHEDULE_SPARSE}[args.schedule]
     if args.config == 5:
-        w = wl.config5(seed=replica_seed(rank), n=args.n)   # replicas: same recipe, rank-specific seed
+        w = wl.config5(seed=replica_seed(0 if args.slab else rank), n=args.n)   # replicas: same recipe, rank-specific seed
         precs = [64, 32] if args.precision == "both" else [int(args.precision)]
         workload = (f"config5 porous medium {args.n}x{args.n} periodic, random disks r~U(8,32) to porosity 0.65, "
                     f"liquid blobs to 50% of pore space, density ratio 1000, viscosity ratio 100, theta=110deg")
@@ -395,6 +496,19 @@ def main():
     # all library work goes to a non-default stream (torch's current stream inside this block): the legacy default
     # stream cannot be captured, and lbm_step replays CUDA graphs on small grids; events are recorded on the same stream
     side = torch.cuda.default_stream() if args.plain_launches else torch.cuda.Stream()
+    if args.slab:
+        if args.config != 5:
+            raise SystemExit("--slab runs config 5 (periodic in y)")
+        with torch.cuda.stream(side):
+            lines = [bench_slab(args, w, p, sched, local, dist, rank, world, workload) for p in precs]
+        if rank == 0:
+            line = lines[0]
+            for p, q in zip(precs[1:], lines[1:]):
+                line[f"fp{p}"] = q
+            print(json.dumps(line), flush=True)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     with torch.cuda.stream(side):
         results = {p: bench_precision(args, w, p, sched, local, dist) for p in precs}
         sweep = {}

@@ -510,6 +510,52 @@ int row_pieces(lbm_ctx* ctx, int j0, int nrows, RowPiece (&pc)[19], int* npc) {
   return LBM_OK;
 }
 
+// lbm_rows_export / lbm_rows_import: the contiguous pieces of some grid rows' state (phi rows, the rows' run in every
+// population plane) to / from one packed buffer, 16 bytes per thread; TO_BUF packs, else unpacks.
+struct RowPieces {
+  char* p[19];
+  unsigned long long end[19];   // running end offset of every piece in the packed buffer, in 16-byte units
+  int n;
+};
+template <bool TO_BUF>
+__global__ void __launch_bounds__(256) k_rows_copy(const RowPieces P, char* __restrict__ buf, unsigned long long total16) {
+  for (unsigned long long t = (unsigned long long)blockIdx.x * 256 + threadIdx.x; t < total16;
+       t += (unsigned long long)gridDim.x * 256) {
+    int k = 0;
+    while (k < P.n - 1 && t >= P.end[k]) k++;
+    const unsigned long long in_piece = t - (k ? P.end[k - 1] : 0ull);
+    uint4* a = reinterpret_cast<uint4*>(P.p[k]) + in_piece;
+    uint4* b = reinterpret_cast<uint4*>(buf) + t;
+    if (TO_BUF) *b = *a;
+    else *a = *b;
+  }
+}
+
+// one launch when every piece is 16-byte aligned (always, unless nx is odd), else one copy per piece
+template <bool TO_BUF>
+int rows_copy(lbm_ctx* ctx, const RowPiece* pc, int n, char* buf) {
+  bool vec = ((uintptr_t)buf & 15) == 0;
+  size_t total = 0;
+  for (int i = 0; i < n; i++) { vec = vec && ((uintptr_t)pc[i].p & 15) == 0 && (pc[i].bytes & 15) == 0; total += pc[i].bytes; }
+  if (vec && total > 0) {
+    RowPieces P;
+    P.n = n;
+    unsigned long long e = 0;
+    for (int i = 0; i < n; i++) { P.p[i] = pc[i].p; e += pc[i].bytes / 16; P.end[i] = e; }
+    const unsigned nb = (unsigned)std::min<unsigned long long>((e + 255) / 256, 148ull * 16);
+    k_rows_copy<TO_BUF><<<nb, 256, 0, ctx->st>>>(P, buf, e);
+    CK(cudaGetLastError());
+    return LBM_OK;
+  }
+  size_t off = 0;
+  for (int i = 0; i < n; i++) {
+    if (TO_BUF) CK(cudaMemcpyAsync(buf + off, pc[i].p, pc[i].bytes, cudaMemcpyDeviceToDevice, ctx->st));
+    else CK(cudaMemcpyAsync(pc[i].p, buf + off, pc[i].bytes, cudaMemcpyDeviceToDevice, ctx->st));
+    off += pc[i].bytes;
+  }
+  return LBM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -996,13 +1042,10 @@ int lbm_rows_export(lbm_ctx* ctx, int32_t j0, int32_t nrows, void* d_buf, size_t
   int n = 0;
   const int rc = row_pieces(ctx, j0, nrows, pc, &n);
   if (rc != LBM_OK) return rc;
-  size_t off = 0;
-  for (int i = 0; i < n; i++) {
-    if (off + pc[i].bytes > cap) return fail(ctx, LBM_ENOMEM, "row buffer too small (lbm_rows_bytes)");
-    CK(cudaMemcpyAsync((char*)d_buf + off, pc[i].p, pc[i].bytes, cudaMemcpyDeviceToDevice, ctx->st));
-    off += pc[i].bytes;
-  }
-  return LBM_OK;
+  size_t need = 0;
+  for (int i = 0; i < n; i++) need += pc[i].bytes;
+  if (need > cap) return fail(ctx, LBM_ENOMEM, "row buffer too small (lbm_rows_bytes)");
+  return rows_copy<true>(ctx, pc, n, (char*)d_buf);
 }
 
 int lbm_rows_import(lbm_ctx* ctx, int32_t j0, int32_t nrows, const void* d_buf, size_t bytes) {
@@ -1014,11 +1057,8 @@ int lbm_rows_import(lbm_ctx* ctx, int32_t j0, int32_t nrows, const void* d_buf, 
   size_t need = 0;
   for (int i = 0; i < n; i++) need += pc[i].bytes;
   if (bytes != need) return fail(ctx, LBM_EINVAL, "row buffer size differs from lbm_rows_bytes: the two contexts do not agree on these rows");
-  size_t off = 0;
-  for (int i = 0; i < n; i++) {
-    CK(cudaMemcpyAsync(pc[i].p, (const char*)d_buf + off, pc[i].bytes, cudaMemcpyDeviceToDevice, ctx->st));
-    off += pc[i].bytes;
-  }
+  const int rc2 = rows_copy<false>(ctx, pc, n, (char*)const_cast<void*>(d_buf));
+  if (rc2 != LBM_OK) return rc2;
   if (ctx->fused) ctx->B_valid = 0;   // B planes kept by lbm_keep_B no longer belong to this state
   return LBM_OK;
 }
