@@ -14,6 +14,8 @@
  *                ghost update phi_G = phi_F / (phi_F + (1 - phi_F) e^eps), eps = -4 dx cos(theta)/W
  *                (Eq. 9, :78-80) }.
  *   lbm_get      rho (:43), phi (A13), u (A14, :313), p (A15, :315) at the current time.
+ *   lbm_rows_export / lbm_rows_import   no arithmetic: the rows of the state next to a cut, for the slab
+ *                decomposition along y (the update of a row reaches 3 rows: A16-A17, R8, :66).
  *
  * Conventions: node (i, j) sits at (x, y) = (i, j); linear index idx = j*nx + i (x fastest);
  * periodic in both directions; flat walls are rows of solid nodes inside the array; dx = dt = 1;
@@ -24,7 +26,8 @@
  * Deviations from the call list SURVEY.md 8(b) proposed (all recorded in DESIGN.md 1): lbm_plan (exact sizing
  * from the mask, needs a device) exists beside lbm_workspace_bytes (host-only upper bound); lbm_params has
  * three more fields (precision, ghost_rule, schedule); B_i are returned only after lbm_keep_B because they
- * are not part of the stored state; test and measurement hooks live in include/lbm_test.h.
+ * are not part of the stored state; lbm_set_populations, lbm_sample_populations and lbm_rows_* were added;
+ * test and measurement hooks live in include/lbm_test.h.
  *
  * Memory and ownership: every pointer is the caller's.  Pointers marked HOST must be host
  * memory (pageable or pinned) and are only used during the call; they are never retained.
