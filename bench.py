@@ -3,7 +3,7 @@
 on BASELINE.json's config 5 (porous medium, density ratio 1000, theta = 110 deg) at 8192^2.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--reps R] [--impl ours|reference] [--config 1..5]
-                    [--n 8192] [--precision 64|32|both] [--schedule auto|baseline|fused|pair|pack|sparse]
+                    [--n 8192] [--precision 64|32|both] [--schedule auto|baseline|fused|pair|pack|sparse|inplace]
                     [--slab [--exchange-every 4]] [--plain-launches] [--no-sweep] [--no-cpu-baseline]
 
 Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement"):
@@ -276,7 +276,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist, steps=None
         dg = sim.diag()
         t_e2e = max_over_ranks([t_e2e], dist, "cuda")[0]
 
-    fused = schedule != binding.SCHEDULE_BASELINE
+    fused = schedule not in (binding.SCHEDULE_BASELINE, binding.SCHEDULE_INPLACE)
     values = 20 if fused else 38
     cls_bytes = 2 if schedule in (binding.SCHEDULE_AUTO, binding.SCHEDULE_PAIR, binding.SCHEDULE_PACK, binding.SCHEDULE_SPARSE) else 1
     bytes_layout = n_fluid * values * rs + cls_bytes * n   # + the class word of every node (cl16: 2 B)
@@ -294,7 +294,7 @@ def bench_precision(args, w, precision, schedule, device_index, dist, steps=None
                   "step_frac_note": "the same algorithmic bytes / the whole timed step (kernel + ghost update), median repetition",
                   "kernel_ms_from": f"CUDA events around every launch of a second run of the same {steps} steps",
                   "clocks_split_run": clocks_split,
-                  "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_FUSED: "k_fused_step", binding.SCHEDULE_SPARSE: "k_fused_sparse"}.get(schedule, "k_fused_pair"),
+                  "traffic": None, "peak_source": peak_src, "kernel": {binding.SCHEDULE_BASELINE: "k_collide_baseline", binding.SCHEDULE_INPLACE: "k_collide_aa_nbr / k_collide_aa_local", binding.SCHEDULE_FUSED: "k_fused_step", binding.SCHEDULE_SPARSE: "k_fused_sparse"}.get(schedule, "k_fused_pair"),
                   "bytes_per_launch": bytes_layout, "values_per_update": values,
                   "kernel_ms": t_collide * 1e3,
                   "layout_copy": None if t_copy is None else {
@@ -445,7 +445,7 @@ def main():
                     help="BASELINE.json config; 5 (the metric's) is the default, 1-4 are the small grids")
     ap.add_argument("--n", type=int, default=8192)
     ap.add_argument("--precision", default="both", choices=["64", "32", "both"])
-    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "pair", "pack", "sparse"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "baseline", "fused", "pair", "pack", "sparse", "inplace"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the 2048^2 / 4096^2 points of config 5")
     ap.add_argument("--plain-launches", action="store_true",
@@ -481,7 +481,8 @@ def main():
         dist = dist_mod
 
     sched = {"auto": binding.SCHEDULE_AUTO, "baseline": binding.SCHEDULE_BASELINE, "fused": binding.SCHEDULE_FUSED,
-             "pair": binding.SCHEDULE_PAIR, "pack": binding.SCHEDULE_PACK, "sparse": binding.SCHEDULE_SPARSE}[args.schedule]
+             "pair": binding.SCHEDULE_PAIR, "pack": binding.SCHEDULE_PACK, "sparse": binding.SCHEDULE_SPARSE,
+             "inplace": binding.SCHEDULE_INPLACE}[args.schedule]
     if args.config == 5:
         w = wl.config5(seed=replica_seed(0 if args.slab else rank), n=args.n)   # replicas: same recipe, rank-specific seed
         precs = [64, 32] if args.precision == "both" else [int(args.precision)]

@@ -76,11 +76,15 @@ enum {
                                  holes (addressed through a 1-bit-per-pair mask + prefix table).  No
                                  dense copy exists: lbm_get / lbm_diag / ... read the compact planes.
                                  Needs even nx, else FUSED is used                                  */
-  LBM_SCHEDULE_SPARSE = 6     /* the PACK layout with lanes mapped to fluid groups: one persistent CTA
+  LBM_SCHEDULE_SPARSE = 6,    /* the PACK layout with lanes mapped to fluid groups: one persistent CTA
                                  per SM, rows brought on chip by 1-D bulk copies (TMA) into a shared-memory
                                  ring, consumer warps work on 32 consecutive entries of the active-group
                                  sequence.  Needs 16-byte groups (fp64: even nx; fp32: nx % 4 == 0) and
                                  at least 4 groups per row, else PACK is used                        */
+  LBM_SCHEDULE_INPLACE = 7    /* single-buffer streaming (AA pattern) on the canonical state: ONE buffer of the
+                                 nine N_i and one of the nine B_i (18 planes instead of BASELINE's 36), one
+                                 thread per node; every thread writes only the slots it read.  Same arithmetic
+                                 and the same two launches per step as BASELINE (collide, phi = sum B_i)    */
 };
 
 typedef struct lbm_ctx lbm_ctx;                 /* opaque; one simulation                         */
@@ -165,7 +169,9 @@ int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B);
  * the grid rows j0 <= j < j0 + nrows (no wrap) into d_buf (DEVICE, >= lbm_rows_bytes bytes, caller-owned),
  * lbm_rows_import overwrites those rows from such a buffer.  The buffer is in the context's own storage format: it
  * can only be imported by a context with the same nx, precision and schedule whose solid mask agrees on these rows
- * (else LBM_EINVAL: the sizes differ).  Asynchronous on the context's stream; lbm_rows_bytes may synchronise once.
+ * (else LBM_EINVAL: the sizes differ).  Under LBM_SCHEDULE_INPLACE the buffer also carries where that schedule parks
+ * the populations at even / odd times: the two contexts must have taken numbers of steps of the same parity since
+ * lbm_init (slabs always have).  Asynchronous on the context's stream; lbm_rows_bytes may synchronise once.
  * Ghost-node geometry is not transferred: each context computes its own at lbm_create. */
 int lbm_rows_bytes(lbm_ctx* ctx, int32_t j0, int32_t nrows, size_t* bytes);
 int lbm_rows_export(lbm_ctx* ctx, int32_t j0, int32_t nrows, void* d_buf, size_t capacity);

@@ -20,6 +20,7 @@ _INC = os.path.join(os.path.dirname(_HERE), "include")
 _SO = os.path.join(_HERE, "liblbm_b200.so")
 
 SCHEDULE_AUTO, SCHEDULE_BASELINE, SCHEDULE_FUSED, SCHEDULE_PAIR, SCHEDULE_PACK, SCHEDULE_SPARSE = 0, 1, 2, 4, 5, 6
+SCHEDULE_INPLACE = 7
 FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
 # include/lbm.h (the product boundary) and include/lbm_test.h (test and measurement hooks)

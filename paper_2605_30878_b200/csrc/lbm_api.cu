@@ -46,6 +46,8 @@ struct lbm_ctx {
   int fused;
   int sched;         // resolved LBM_SCHEDULE_* (never AUTO)
   int keep_B;
+  int inplace;       // INPLACE schedule: one N and one B buffer, AA pattern
+  int aa_local;      // ... and the state is parked in the nodes' own opposite slots (odd number of steps since standard)
   int B_owned;       // compacted layouts: the B planes are not in the workspace; lbm_keep_B allocates them on demand
   int B_valid;       // B planes of buffer `cur` hold the post-collision B* of the last step
   cudaStream_t st;
@@ -138,7 +140,7 @@ int validate(const lbm_params* P, const char** why) {
   if (!(P->theta_deg >= 0.0 && P->theta_deg <= 180.0)) { *why = "theta outside [0, 180]"; return LBM_EINVAL; }
   if (!(P->mobility > 0.0 && P->mobility < 0.3)) { *why = "mobility outside (0, 0.3)"; return LBM_EINVAL; }
   if (P->ghost_rule != 0 && P->ghost_rule != 1) { *why = "ghost_rule must be 0 or 1"; return LBM_EINVAL; }
-  if (P->schedule < 0 || P->schedule > 6 || P->schedule == 3) { *why = "unknown schedule"; return LBM_EINVAL; }
+  if (P->schedule < 0 || P->schedule > 7 || P->schedule == 3) { *why = "unknown schedule"; return LBM_EINVAL; }
   if (P->wall_rows != 0 && P->wall_rows != 1) { *why = "wall_rows must be 0 or 1"; return LBM_EINVAL; }
   return LBM_OK;
 }
@@ -191,7 +193,9 @@ void build_disk_cells(const lbm_params* P, const lbm_disk* disks, int n_disks, i
   for (size_t k = 0; k < cells.size(); k++) std::copy(cells[k].begin(), cells[k].end(), list.begin() + start[k]);
 }
 
-bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELINE; }
+bool use_inplace(const lbm_params* P) { return P->schedule == LBM_SCHEDULE_INPLACE; }
+// the B_i are part of the stored state under BASELINE and INPLACE (the canonical 36 / 18 + 18 values)
+bool use_fused(const lbm_params* P) { return P->schedule != LBM_SCHEDULE_BASELINE && !use_inplace(P); }
 
 // one layout function serves both sizing (base == nullptr) and carving; everything that does not
 // depend on the ghost count comes first, so a carve with ng = 0 and one with the real ng agree
@@ -254,10 +258,11 @@ size_t layout(lbm_ctx* c, char* base, const lbm_params* P, long long ng, long lo
     Nc1 = A.take<char>(9 * cps * G * rs);
     ptab = A.take<uint2>((size_t)P->ny * nw);
   } else {
+    const bool single = use_inplace(P);   // INPLACE: one buffer of N and one of B
     N0 = A.take<char>(9 * ps * rs);
-    N1 = A.take<char>(9 * ps * rs);
+    N1 = single ? nullptr : A.take<char>(9 * ps * rs);
     B0 = A.take<char>(9 * ps * rs);
-    B1 = fused ? nullptr : A.take<char>(9 * ps * rs);
+    B1 = (fused || single) ? nullptr : A.take<char>(9 * ps * rs);
   }
   char* p0 = A.take<char>(n * rs);
   char* p1 = A.take<char>(n * rs);
@@ -321,6 +326,7 @@ Consts<R> make_consts(const lbm_params& P) {
   C.E = (R)exp(eps); C.eps = (R)eps;
   C.phi_solid = (R)(0.5 * (1.0 + ct));
   C.ghost_rule = P.ghost_rule;
+  C.all_links = 0;
   return C;
 }
 
@@ -348,6 +354,12 @@ void launch_ghost(lbm_ctx* c) {
 bool launch_fused_sparse(lbm_ctx* c, const Consts<double>& C, const double* Ns, double* Nd, double* Bd, const double* pi, double* po);
 bool launch_fused_sparse(lbm_ctx* c, const Consts<float>& C, const float* Ns, float* Nd, float* Bd, const float* pi, float* po);
 
+// INPLACE: where the state is parked (lbm_kernels.cuh, k_collide_aa_*); the readers get it through Consts::all_links
+void set_parking(lbm_ctx* c, bool local) {
+  c->aa_local = local ? 1 : 0;
+  c->Cd.all_links = c->Cf.all_links = c->aa_local;
+}
+
 struct StepTimer {   // optional event brackets around each launch (lbm_step_timed): 4 events per step, read in bulk
   cudaEvent_t* ev;   // the caller provides 4 events for this step
 };
@@ -358,7 +370,19 @@ int step_once(lbm_ctx* c, bool write_B, StepTimer* tm = nullptr) {
   if (tm) cudaEventRecord(tm->ev[0], c->st);
   const dim3 grid = row_grid(c->P.nx, c->P.ny, &bx);
   const Consts<R>& C = consts_of<R>(c);
-  if (!c->fused) {
+  if (c->inplace) {   // AA pattern on the single N / B buffers (cur stays 0); phi ping-pongs as everywhere
+    if (!c->aa_local)
+      k_collide_aa_nbr<R><<<grid, bx, 0, c->st>>>(C, c->cls, c->links, (R*)c->N[0], (R*)c->B[0], (const R*)c->phi[c->pcur]);
+    else
+      k_collide_aa_local<R><<<grid, bx, 0, c->st>>>(C, c->cls, (R*)c->N[0], (R*)c->B[0], (const R*)c->phi[c->pcur]);
+    set_parking(c, !c->aa_local);
+    c->pcur ^= 1;
+    if (tm) cudaEventRecord(tm->ev[1], c->st);
+    k_phi_sum<R><<<grid, bx, 0, c->st>>>(consts_of<R>(c), c->cls, c->links, (const R*)c->B[0], (R*)c->phi[c->pcur]);
+    c->launches[0]++;
+    c->launches[1]++;
+    c->B_valid = 1;
+  } else if (!c->fused) {
     k_collide_baseline<R><<<grid, bx, 0, c->st>>>(C, c->cls, c->links, (const R*)c->N[c->cur],
                                                  (R*)c->N[c->cur ^ 1], (R*)c->B[c->cur ^ 1],
                                                  (const R*)c->phi[c->pcur]);
@@ -627,6 +651,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   c->n = n;
   c->is32 = prm->precision == 32;
   c->fused = use_fused(prm) ? 1 : 0;
+  c->inplace = use_inplace(prm) ? 1 : 0;
   c->sched = prm->schedule == LBM_SCHEDULE_AUTO ? (use_pack(prm) ? LBM_SCHEDULE_PACK : LBM_SCHEDULE_PAIR) : prm->schedule;
   if (c->sched == LBM_SCHEDULE_SPARSE && !use_sparse(prm)) c->sched = use_pack(prm) ? LBM_SCHEDULE_PACK : LBM_SCHEDULE_PAIR;
   c->st = (cudaStream_t)cuda_stream;
@@ -832,6 +857,7 @@ int lbm_init(lbm_ctx* ctx, const double* phi0, const double* u0) {
   ctx->cur = 0;
   ctx->pcur = 0;
   ctx->t = 0;
+  set_parking(ctx, false);   // k_init writes the standard parking
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
   ctx->ccur = 0;
@@ -859,7 +885,7 @@ int lbm_step(lbm_ctx* ctx, int64_t nsteps) {
   if (!ctx || nsteps < 0) return fail(ctx, LBM_EINVAL, "bad argument");
   int64_t s = 0;
   // the legacy default stream cannot be captured; with keep_B the last step differs from the others
-  if (ctx->st != nullptr && ctx->st != cudaStreamLegacy && !ctx->keep_B && ctx->n <= kGraphMaxNodes) {
+  if (ctx->st != nullptr && ctx->st != cudaStreamLegacy && !ctx->keep_B && !ctx->inplace && ctx->n <= kGraphMaxNodes) {
     if (!ctx->graph_warm && nsteps - s >= kGraphSteps + 2) {   // first launches outside any capture
       for (int k = 0; k < 2; k++, s++)
         if ((ctx->is32 ? step_once<float>(ctx, false) : step_once<double>(ctx, false)) != LBM_OK)
@@ -1069,6 +1095,30 @@ int lbm_set_populations(lbm_ctx* ctx, const double* N, const double* B) {
   const size_t n = ctx->n;
   int bx;
   const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  if (ctx->inplace && ctx->aa_local) {
+    // k_scatter_plane writes the standard parking: bring what is NOT overwritten there first.  A direction and its
+    // opposite only ever use each other's planes, so pair by pair: gather both (as the readers see them), scatter both.
+    for (int which = 0; which < 2; which++) {
+      if (which ? B != nullptr : N != nullptr) continue;
+      const int pairs[4][2] = {{1, 3}, {2, 4}, {5, 7}, {6, 8}};
+      for (const auto& pr : pairs) {
+        for (int t = 0; t < 2; t++) {
+          double* dst = ctx->stage + (size_t)t * n;
+          if (ctx->is32) k_gather_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, which ? B_view<float>(ctx) : pop_view<float>(ctx), pr[t], 0.0, dst);
+          else k_gather_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, which ? B_view<double>(ctx) : pop_view<double>(ctx), pr[t], 0.0, dst);
+        }
+        for (int t = 0; t < 2; t++) {
+          const double* src = ctx->stage + (size_t)t * n;
+          if (ctx->is32) k_scatter_plane<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, src, pr[t], 0.0, which ? B_view<float>(ctx) : pop_view<float>(ctx));
+          else k_scatter_plane<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, src, pr[t], 0.0, which ? B_view<double>(ctx) : pop_view<double>(ctx));
+        }
+        ctx->launches[3] += 4;
+      }
+      CK(cudaGetLastError());
+    }
+    CK(cudaStreamSynchronize(ctx->st));
+    set_parking(ctx, false);
+  }
   const double chi[9] = {ctx->Cd.chi0, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1, ctx->Cd.chi1,
                          ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5, ctx->Cd.chi5};
   void* Bp = ctx->fused ? ctx->B[0] : ctx->B[ctx->cur];   // may be absent (compacted layout without lbm_keep_B)
@@ -1181,6 +1231,7 @@ int lbm_diag(lbm_ctx* ctx, double out[8]) {
 int lbm_layout_copy_timed(lbm_ctx* ctx, int32_t iters, double* ms_per_pass) {
   if (!ctx || iters < 1 || !ms_per_pass) return fail(ctx, LBM_EINVAL, "bad argument");
   if (ctx->packed) return fail(ctx, LBM_EINVAL, "the dense SoA layout this helper measures is not kept under PACK / SPARSE; create the context with LBM_SCHEDULE_PAIR");
+  if (ctx->inplace) return fail(ctx, LBM_EINVAL, "an INPLACE context has no second buffer to copy into; create the context with LBM_SCHEDULE_PAIR");
   const size_t rs = ctx->is32 ? 4 : 8, nps = 32 / rs;
   if (ctx->n % nps != 0 || ctx->Cd.ps % nps != 0) return fail(ctx, LBM_EINVAL, "nx*ny is not a whole number of 32-byte sectors");
   const size_t nsec = ctx->n / nps, psec = ctx->Cd.ps / nps;

@@ -413,6 +413,13 @@ __device__ __forceinline__ void load_phi9(const R* __restrict__ phi, const Nbr& 
   for (int q = 0; q < 9; q++) ph[q] = phi[b.dst[q]];
 }
 
+// link bits of a node as the readers of the state see them (see Consts::all_links)
+template <typename R>
+__device__ __forceinline__ unsigned link_bits(const Consts<R>& C, unsigned c, const uint8_t* __restrict__ links, int k) {
+  if (C.all_links) return 0xffu;
+  return (c == 1) ? links[k] : 0u;
+}
+
 // ------------------------------------------------------------------------------------------
 // BASELINE schedule, kernel (3): fused pull-stream + collide, one thread per node.
 // Reads 9 pulled N, the 3x3 phi neighbourhood, 1 class byte; writes 9 N* and 9 B*.
@@ -455,13 +462,74 @@ __global__ void __launch_bounds__(256) k_phi_sum(const Consts<R> C, const uint8_
   const uint8_t c = cls[k];
   if (c >= 2) return;
   const Nbr b = make_nbr(i, j, C.nx, C.ny);
-  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const unsigned lk = link_bits(C, c, links, k);
   R v[9];
   pull9<R>(Bsrc, n, k, b, lk, v);
   R s = v[0];
 #pragma unroll
   for (int q = 1; q < 9; q++) s += v[q];
   phi[k] = s;
+}
+
+// ------------------------------------------------------------------------------------------
+// INPLACE schedule (f4: single-buffer streaming, the AA pattern): the canonical state N_i, B_i in ONE buffer each.
+// Every thread writes only the slots it read, so no other thread's input is ever overwritten and the launch order
+// does not matter.  The stored value is, as everywhere, the post-collision population; where it is parked alternates:
+//   even time ("standard"): N_q*(y) in slot q of y; the reader at x pulls slot q of x - c_q (own slot opp(q) on a link);
+//   odd time  ("local"):    N_q*(y) in slot opp(q) of y + c_q (in slot q of y itself if y + c_q is solid): the reader
+//                           at x finds all nine in its own opposite slots.
+// k_collide_aa_nbr takes standard to local, k_collide_aa_local takes local to standard.  The collision never reads
+// B_i, so the B planes simply follow the same parking rule (k_phi_sum reads them afterwards).
+// ------------------------------------------------------------------------------------------
+template <typename R>
+__global__ void __launch_bounds__(256) k_collide_aa_nbr(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                        const uint8_t* __restrict__ links, R* __restrict__ N,
+                                                        R* __restrict__ B, const R* __restrict__ phi) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = C.ps;
+  const int k = j * C.nx + i;
+  const uint8_t c = cls[k];
+  if (c >= 2) return;
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  const unsigned lk = (c == 1) ? links[k] : 0u;
+  R nn[9], ph[9], ns[9], bs[9];
+  load_phi9<R>(phi, b, ph);
+  pull9<R>(N, n, k, b, lk, nn);
+  node_update<R, true>(C, nn, ph, ns, bs, nullptr);
+  N[k] = ns[0];
+  B[k] = bs[0];
+#pragma unroll
+  for (int q = 1; q < 9; q++) {
+    // towards x + c_q = x - c_opp(q): the slot nn[opp(q)] was read from; a solid node there sends it back (R12)
+    const bool back = (lk >> (opp(q) - 1)) & 1u;
+    const size_t dst = back ? (size_t)q * n + k : (size_t)opp(q) * n + b.src[opp(q)];
+    N[dst] = ns[q];
+    B[dst] = bs[q];
+  }
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) k_collide_aa_local(const Consts<R> C, const uint8_t* __restrict__ cls,
+                                                          R* __restrict__ N, R* __restrict__ B,
+                                                          const R* __restrict__ phi) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+  if (i >= C.nx) return;
+  const size_t n = C.ps;
+  const int k = j * C.nx + i;
+  if (cls[k] >= 2) return;
+  const Nbr b = make_nbr(i, j, C.nx, C.ny);
+  R nn[9], ph[9], ns[9], bs[9];
+  load_phi9<R>(phi, b, ph);
+  nn[0] = N[k];
+#pragma unroll
+  for (int q = 1; q < 9; q++) nn[q] = N[(size_t)opp(q) * n + k];
+  node_update<R, true>(C, nn, ph, ns, bs, nullptr);
+#pragma unroll
+  for (int q = 0; q < 9; q++) {
+    N[(size_t)q * n + k] = ns[q];
+    B[(size_t)q * n + k] = bs[q];
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -550,7 +618,7 @@ __global__ void __launch_bounds__(256) k_moments(const Consts<R> C, const uint8_
     return;
   }
   const Nbr b = make_nbr(i, j, C.nx, C.ny);
-  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const unsigned lk = link_bits(C, c, links, k);
   R nn[9], ph[9], ns[9], bs[9];
   NodeOut<R> o;
   load_phi9<R>(phi, b, ph);
@@ -575,7 +643,7 @@ __global__ void __launch_bounds__(256) k_gather_plane(const Consts<R> C, const u
   const uint8_t c = cls[k];
   if (c >= 2) { out[k] = 0.0; return; }
   const Nbr b = make_nbr(i, j, C.nx, C.ny);
-  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const unsigned lk = link_bits(C, c, links, k);
   R v;
   if (q == 0) v = pop.at(0, k);
   else v = ((lk >> (q - 1)) & 1u) ? pop.at(opp(q), k) : pop.at(q, b.src[q]);
@@ -630,7 +698,7 @@ __global__ void __launch_bounds__(128) k_gather_samples(const Consts<R> C, const
   const int k = (int)idx[t];
   const uint8_t c = cls[k];
   const Nbr b = make_nbr(k % C.nx, k / C.nx, C.nx, C.ny);
-  const unsigned lk = (c == 1) ? links[k] : 0u;
+  const unsigned lk = link_bits(C, c, links, k);
   const double chi[9] = {(double)C.chi0, (double)C.chi1, (double)C.chi1, (double)C.chi1, (double)C.chi1,
                          (double)C.chi5, (double)C.chi5, (double)C.chi5, (double)C.chi5};
   for (int q = 0; q < 9; q++) {
@@ -701,7 +769,7 @@ __global__ void __launch_bounds__(256) k_diag_partial(const Consts<R> C, const u
     const uint8_t c = cls[k];
     if (c < 2) {
       const Nbr b = make_nbr(i, j, C.nx, C.ny);
-      const unsigned lk = (c == 1) ? links[k] : 0u;
+      const unsigned lk = link_bits(C, c, links, k);
       R nn[9], ph[9], ns[9], bs[9];
       NodeOut<R> o;
       load_phi9<R>(phi, b, ph);

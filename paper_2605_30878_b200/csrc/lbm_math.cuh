@@ -32,6 +32,8 @@ struct Consts {
   R E, eps;             // e^eps and eps = -(4/W) cos(theta) of Eq. 9           (:78-80)
   R phi_solid;          // (1 + cos theta)/2                                     (:100)
   int ghost_rule;
+  int all_links;        // INPLACE schedule at odd times: every population a node pulls sits in the node's own opposite
+                        // slot, which is what the readers do for a bounce-back link
 };
 
 __device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }

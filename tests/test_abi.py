@@ -74,3 +74,13 @@ def test_workspace_bytes_is_host_only_and_monotone():
     assert binding.workspace_bytes(binding.LBMParams(nx=64, ny=48, precision=32), 1000) < b
     assert binding.workspace_bytes(binding.LBMParams(nx=2, ny=48), 10) == 0          # nx < 3
     assert binding.workspace_bytes(binding.LBMParams(nx=64, ny=48, W=3.0), 10) == 0   # W < 4
+
+
+def test_inplace_schedule_keeps_one_buffer_of_each_population_set():
+    """INPLACE (f4, single-buffer streaming): 18 population planes in the workspace where BASELINE has 36."""
+    nx, ny = 512, 384
+    for prec, rs in ((64, 8), (32, 4)):
+        base = binding.workspace_bytes(binding.LBMParams(nx=nx, ny=ny, precision=prec, schedule=binding.SCHEDULE_BASELINE), 5000)
+        inpl = binding.workspace_bytes(binding.LBMParams(nx=nx, ny=ny, precision=prec, schedule=binding.SCHEDULE_INPLACE), 5000)
+        saved = base - inpl
+        assert 18 * nx * ny * rs <= saved <= 18 * (nx * ny + 4096) * rs + 18 * 256

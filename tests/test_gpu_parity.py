@@ -13,9 +13,10 @@ from paper_2605_30878_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-BASELINE, FUSED, PAIR, PACK, SPARSE = 1, 2, 4, 5, 6
+BASELINE, FUSED, PAIR, PACK, SPARSE, INPLACE = 1, 2, 4, 5, 6, 7
 SCHEDULES = [pytest.param(BASELINE, id="baseline"), pytest.param(FUSED, id="fused"),
-             pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack"), pytest.param(SPARSE, id="sparse")]
+             pytest.param(PAIR, id="pair"), pytest.param(PACK, id="pack"), pytest.param(SPARSE, id="sparse"),
+             pytest.param(INPLACE, id="inplace")]
 
 
 # ---- local update of single nodes ---------------------------------------------------------------
@@ -532,7 +533,8 @@ def test_config5_8192_is_deterministic():
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
 
 
-@pytest.mark.parametrize("schedule", [pytest.param(0, id="auto"), pytest.param(BASELINE, id="baseline"), pytest.param(SPARSE, id="sparse")])
+@pytest.mark.parametrize("schedule", [pytest.param(0, id="auto"), pytest.param(BASELINE, id="baseline"), pytest.param(SPARSE, id="sparse"),
+                                      pytest.param(INPLACE, id="inplace")])
 def test_set_populations_round_trip_and_restart(schedule):
     """lbm_set_populations: (i) what is set is what lbm_get_populations returns, (ii) both sides handed the
     same far-from-equilibrium state continue identically, (iii) a fresh context restarted from another
@@ -562,9 +564,17 @@ def test_set_populations_round_trip_and_restart(schedule):
     g2.step(2); o2.step(2)
     err2, _ = field_errors(g2, o2)
     assert max(err2.values()) < 1e-11, err2
-    # restart: N only (phi and the ghost values of the receiving context stay as they are)
+    # restart: N only (phi and the ghost values of the receiving context stay as they are).  g has taken an odd number of
+    # steps: under INPLACE its state is parked in the nodes' own slots and the B_i must be re-parked, not lost
+    B_before = g.get_populations(want_B=True)[1] if schedule in (BASELINE, INPLACE) else None
     g.set_populations(N=N2)
     assert np.abs(g.get_populations(want_B=False)[0] - N2)[:, fluid].max() <= 1e-15
+    if B_before is not None:
+        assert np.array_equal(g.get_populations(want_B=True)[1], B_before)
+        o.set_populations(N2, B_before)
+        g.step(3); o.step(3)
+        eN, eB = pop_errors(g, o, fluid)
+        assert eN < 1e-13 and eB < 1e-13, (eN, eB)
 
 
 def test_symmetric_setup_differs_only_where_the_gradient_vanishes():

@@ -186,7 +186,7 @@ def _slabbed(w, precision, schedule, steps, disks, world, k):
 
 
 SCHED = [pytest.param(0, id="auto"), pytest.param(binding.SCHEDULE_BASELINE, id="baseline"),
-         pytest.param(binding.SCHEDULE_SPARSE, id="sparse")]
+         pytest.param(binding.SCHEDULE_SPARSE, id="sparse"), pytest.param(binding.SCHEDULE_INPLACE, id="inplace")]
 
 
 def _assert_close(got, want, precision, what):
@@ -244,11 +244,11 @@ def test_gpu_slabs_without_exchange_differ():
 @pytest.mark.gpu
 def test_rows_export_import_round_trip_and_errors():
     w = wl.config5(seed=1, n=256)
-    for schedule in (0, binding.SCHEDULE_FUSED, binding.SCHEDULE_SPARSE, binding.SCHEDULE_BASELINE):
+    for schedule in (0, binding.SCHEDULE_FUSED, binding.SCHEDULE_SPARSE, binding.SCHEDULE_BASELINE, binding.SCHEDULE_INPLACE):
         a = binding.LBM(binding.LBMParams(precision=64, schedule=schedule, **w.param_dict()), w.mask, w.disks)
         b = binding.LBM(binding.LBMParams(precision=64, schedule=schedule, **w.param_dict()), w.mask, w.disks)
         a.init(w.phi0); b.init(w.phi0)
-        a.step(6); b.step(3)
+        a.step(6); b.step(4 if schedule == binding.SCHEDULE_INPLACE else 3)   # INPLACE: same parity of steps (lbm.h)
         nb = a.rows_bytes(0, w.ny)
         assert nb == sum(a.rows_bytes(j, 32) for j in range(0, w.ny, 32))      # the pieces add up
         buf = torch.empty(nb, dtype=torch.uint8, device="cuda")
