@@ -26,7 +26,8 @@
  * Deviations from the call list SURVEY.md 8(b) proposed (all recorded in DESIGN.md 1): lbm_plan (exact sizing
  * from the mask, needs a device) exists beside lbm_workspace_bytes (host-only upper bound); lbm_params has
  * three more fields (precision, ghost_rule, schedule); B_i are returned only after lbm_keep_B because they
- * are not part of the stored state; lbm_set_populations, lbm_sample_populations and lbm_rows_* were added;
+ * are not part of the stored state; lbm_set_populations, lbm_sample_populations, lbm_rows_* and lbm_diag_static
+ * were added;
  * test and measurement hooks live in include/lbm_test.h.
  *
  * Memory and ownership: every pointer is the caller's.  Pointers marked HOST must be host
@@ -202,6 +203,17 @@ int lbm_get_classification(lbm_ctx* ctx, uint8_t* cls, int32_t* n_ghost, int32_t
  * deterministic): out[0] = sum phi, [1] = sum (1 - phi), [2] = 1/2 sum rho |u|^2, [3] = max |u|,
  * [4] = min phi, [5] = max phi, [6] = number of fluid nodes, [7] = 1 if any NaN.  out: HOST. */
 int lbm_diag(lbm_ctx* ctx, double out[8]);
+
+/* The same diagnostics for callers that cannot allocate or synchronise (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the eight values of lbm_diag go to d_out (DEVICE, 8 doubles, caller-owned),
+ * asynchronously on the context's stream.  The block partials of the reduction live in a file-scope device array of
+ * the library (4 MiB, held by every GPU that loads the library until the process exits) instead of the workspace; the
+ * call makes no cudaMalloc / cudaFree, no host copy and no synchronisation.
+ * Limit: ceil(nx / 256) * ny <= 65,536 block partials (e.g. up to 4096 x 4096); larger grids get LBM_EINVAL with the
+ * numbers in lbm_last_error: use lbm_diag there.  The array is shared by ALL contexts on a device and keeps the last
+ * call's partials (every slot that is read is written first, nothing needs clearing): two calls that overlap on the
+ * GPU (different streams, or graphs launched concurrently) race; calls on one stream, or otherwise ordered, do not. */
+int lbm_diag_static(lbm_ctx* ctx, double* d_out);
 
 const char* lbm_last_error(const lbm_ctx* ctx); /* ctx may be NULL: last error of lbm_plan/create */
 const char* lbm_version(void);

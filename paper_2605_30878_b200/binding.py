@@ -27,7 +27,7 @@ FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 EXPORTS = ("lbm_plan", "lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
            "lbm_get_populations", "lbm_set_populations", "lbm_rows_bytes", "lbm_rows_export", "lbm_rows_import",
            "lbm_keep_B", "lbm_sample_populations",
-           "lbm_get_classification", "lbm_diag", "lbm_last_error", "lbm_version", "lbm_destroy")
+           "lbm_get_classification", "lbm_diag", "lbm_diag_static", "lbm_last_error", "lbm_version", "lbm_destroy")
 TEST_EXPORTS = ("lbm_node_update_batch", "lbm_step_timed", "lbm_layout_copy_timed", "lbm_launch_counts")
 
 
@@ -123,6 +123,7 @@ def load_library() -> C.CDLL:
         L.lbm_sample_populations.argtypes = [vp, i64, vp, vp, vp]
         L.lbm_get_classification.argtypes = [vp] * 9
         L.lbm_diag.argtypes = [vp, vp]
+        L.lbm_diag_static.argtypes = [vp, vp]
         L.lbm_node_update_batch.argtypes = [C.POINTER(_Params), i64, vp, vp, vp, vp, vp]
         L.lbm_launch_counts.argtypes = [vp, vp, C.c_int32]
         L.lbm_last_error.argtypes = [vp]
@@ -312,6 +313,11 @@ class LBM:
         _check(load_library().lbm_diag(self._h, out.ctypes.data), self._h)
         return dict(sum_phi=out[0], sum_1mphi=out[1], ke=out[2], umax=out[3], phi_min=out[4],
                     phi_max=out[5], n_fluid=out[6], nan=out[7])
+
+    def diag_static(self, out_ptr: int):
+        """lbm_diag without allocation, host copy or synchronisation: the eight values go to a DEVICE buffer of 8 doubles
+        (asynchronous on the stream); the reduction's scratch is a static device array of the library (lbm.h: limits)."""
+        _check(load_library().lbm_diag_static(self._h, int(out_ptr)), self._h)
 
     def launch_counts(self, reset: bool = False):
         out = np.zeros(4, np.int64)

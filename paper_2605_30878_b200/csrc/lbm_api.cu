@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -104,8 +105,18 @@ struct lbm_ctx {
   int graph_warm;          // two plain steps have run on this context (kernel attributes are set)
   cudaGraphExec_t gexec[8];
   int64_t gdelta[8][4];   // launches a replay adds
+  // lbm_diag_static: device address of g_diag_static on this context's device, resolved at lbm_create
+  DiagVec* diag_static;
+  int diag_static_err;     // cudaError_t of that resolution
   char err[512];
 };
+
+// ---- scratch of lbm_diag_static (lbm.h): the block partials of the diagnostics reduction in a file-scope device
+// array, so that the call needs no workspace region, no cudaMalloc and no host synchronisation.  Every GPU that loads
+// the library holds these 4 MiB until the process exits.  In host code the NAME is a host-side stand-in, not a device
+// address: the address a kernel can use comes from cudaGetSymbolAddress (static_scratch_of below).
+constexpr long long kDiagStaticMax = 65536;   // block partials (64 B each): grids up to e.g. 4096 x 4096
+static __device__ __align__(256) DiagVec g_diag_static[kDiagStaticMax];
 
 namespace {
 
@@ -126,6 +137,26 @@ int cuda_fail(lbm_ctx* c, cudaError_t e, const char* where) {
     cudaError_t e_ = (call);                                       \
     if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
   } while (0)
+
+// once per device, with that device current (lbm_create is the set-up): the device address of g_diag_static
+cudaError_t static_scratch_of(DiagVec** ptr) {
+  struct Entry { int dev; DiagVec* p; cudaError_t e; };
+  static std::mutex mu;
+  static std::vector<Entry> table;
+  *ptr = nullptr;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lk(mu);
+  for (const auto& t : table)
+    if (t.dev == dev) { *ptr = t.p; return t.e; }
+  void* p = nullptr;
+  e = cudaGetSymbolAddress(&p, g_diag_static);
+  if (e != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+  table.push_back(Entry{dev, (DiagVec*)p, e});
+  *ptr = (DiagVec*)p;
+  return e;
+}
 
 int validate(const lbm_params* P, const char** why) {
   *why = "";
@@ -834,6 +865,7 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   }
   CKC(cudaStreamSynchronize(c->st));
 #undef CKC
+  c->diag_static_err = (int)static_scratch_of(&c->diag_static);   // a failure is reported by lbm_diag_static, not here
   *out = c;
   return LBM_OK;
 }
@@ -1225,6 +1257,38 @@ int lbm_diag(lbm_ctx* ctx, double out[8]) {
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(out, ctx->diag_out, 8 * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
   CK(cudaStreamSynchronize(ctx->st));
+  return LBM_OK;
+}
+
+int lbm_diag_static(lbm_ctx* ctx, double* d_out) {
+  if (!ctx || !d_out) return fail(ctx, LBM_EINVAL, "null argument");
+  if (!ctx->diag_static) {
+    char buf[300];
+    snprintf(buf, sizeof buf, "lbm_diag_static: cudaGetSymbolAddress of the static scratch failed at lbm_create: %s",
+             cudaGetErrorString((cudaError_t)ctx->diag_static_err));
+    return fail(ctx, LBM_ECUDA, buf);
+  }
+  int bx;
+  const dim3 grid = row_grid(ctx->P.nx, ctx->P.ny, &bx);
+  const long long m = (long long)grid.x * grid.y;
+  if (m > kDiagStaticMax) {
+    char buf[300];
+    snprintf(buf, sizeof buf, "lbm_diag_static: this grid needs %lld block partials, the static scratch holds %lld "
+             "(ceil(nx / 256) * ny must not exceed it); use lbm_diag", m, kDiagStaticMax);
+    return fail(ctx, LBM_EINVAL, buf);
+  }
+  // every one of the m slots is written by its block before k_diag_final reads slots 0 .. m-1: whatever an earlier
+  // call left in the array is never read, nothing has to be cleared
+  DiagVec* part = ctx->diag_static;
+  if (ctx->is32)
+    k_diag_partial<float><<<grid, bx, 0, ctx->st>>>(ctx->Cf, ctx->cls, ctx->links, pop_view<float>(ctx),
+                                                    (const float*)ctx->phi[ctx->pcur], part);
+  else
+    k_diag_partial<double><<<grid, bx, 0, ctx->st>>>(ctx->Cd, ctx->cls, ctx->links, pop_view<double>(ctx),
+                                                     (const double*)ctx->phi[ctx->pcur], part);
+  k_diag_final<<<1, 1024, 0, ctx->st>>>(part, m, d_out);
+  ctx->launches[3] += 2;
+  CK(cudaGetLastError());
   return LBM_OK;
 }
 
