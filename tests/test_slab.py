@@ -262,3 +262,14 @@ def test_rows_export_import_round_trip_and_errors():
         with pytest.raises(binding.LBMError):
             b.rows_import(0, 16, buf.data_ptr(), nb)                            # size of other rows
         a.close(); b.close()
+
+
+@pytest.mark.gpu
+def test_gpu_slabs_config5_4096_two_slabs():
+    """The size of the sweep's middle point (16.8 M nodes, compact planes of several hundred MB): two slabs with the
+    analytic disk list against the single-domain run."""
+    w = wl.config5(seed=0, n=4096)
+    want = _whole(w, 32, 0, 8, w.disks)
+    got, (H, nl) = _slabbed(w, 32, 0, 8, w.disks, 2, 4)
+    assert nl == 2048 + 2 * H
+    _assert_close(got, want, 32, "4096")
