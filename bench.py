@@ -52,7 +52,7 @@ def measured_peak():
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,clocks.mem,power.draw,power.limit")
 
     def __init__(self, index: int):
         self.index, self.proc, self.path = index, None, f"/tmp/lbm_clocks_{os.getpid()}_{index}.csv"
@@ -77,7 +77,7 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         self.fh.close()
-        sm, mx, reasons = [], [], set()
+        sm, mx, mem, pw, pl, reasons = [], [], [], [], [], set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
         try:
             for line in open(self.path):
@@ -91,11 +91,17 @@ class ClockSampler:
                 for nm, v in zip(names, parts[2:6]):
                     if v.lower().startswith("active"):
                         reasons.add(nm)
+                try:   # memory clock and board power: context for the sw_power_cap reason (optional columns)
+                    mem.append(float(parts[6])); pw.append(float(parts[7])); pl.append(float(parts[8]))
+                except (ValueError, IndexError):
+                    pass
             os.remove(self.path)
         except Exception:
             pass
         if sm:
             out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+        if mem:
+            out.update(mem_mhz=float(np.median(mem)), power_w=float(np.median(pw)), power_limit_w=float(max(pl)))
         out["reasons"] = sorted(reasons)
         return out
 
