@@ -671,9 +671,6 @@ int lbm_create(lbm_ctx** out, const lbm_params* prm, const uint8_t* mask, const 
   const size_t min_ws = layout(nullptr, nullptr, prm, 0, nfp);
   if (workspace_bytes < min_ws) return fail(nullptr, LBM_ENOMEM, "workspace too small");
 
-#ifdef LBM_L2_FETCH
-  cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, LBM_L2_FETCH);   // tuning experiment
-#endif
   lbm_ctx* c = new (std::nothrow) lbm_ctx;
   if (!c) return fail(nullptr, LBM_ENOMEM, "host allocation failed");
   memset(c, 0, sizeof *c);
