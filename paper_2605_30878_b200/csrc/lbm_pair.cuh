@@ -515,11 +515,12 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   constexpr int OUTC = 30 * LaneOf<V>::NL;
   const int nwx = (C.nx + OUTC - 1) / OUTC;
   const int gx = (nwx + WARPS - 1) / WARPS;
-  // Rows per warp march.  Long marches amortise the two halo rows and the pipeline fill (about 5 rows' worth); short
-  // ones make more CTAs.  A launch takes about waves x (TY + 5) row times, waves = ceil(CTAs / resident CTAs of the
-  // device): take the TY that minimises it; marches longer than 16 rows only when they still fill the device once
-  // (a single under-filled wave of long marches lost to three waves of short ones: measured on 1024^2 ... 8192^2
-  // and the paper's 1500 x 900, profiles/r2_small_grids.md).
+  // Rows per warp march.  Long marches amortise the two halo rows and the pipeline fill (about 6 rows' worth); short
+  // ones make more CTAs.  The CTAs of a launch run in waves of `slots` (every resident warp takes about as long per row
+  // whether the SM is full or not), so a launch takes about ceil(CTAs / slots) x (TY + 6) row times: take the TY that
+  // minimises it.  What matters on mid-size grids is that the last wave is full: 2048^2 runs 10-12 % faster with the
+  // march length that fits the grid into exactly one wave (41 rows in fp64, 21 in fp32) than with a power of two
+  // (profiles/r2_small_grids.md).
   int nsm = 148;
   {
     int dev = 0;
@@ -528,10 +529,9 @@ bool launch_fused_lane(const Consts<typename LaneOf<V>::R>& C, const uint16_t* c
   const long long slots = (long long)nsm * MINB;
   int TY = LBM_PAIR_TY;
   long long best = -1;
-  for (int t = LBM_PAIR_TY; t >= 8; t >>= 1) {
+  for (int t = LBM_PAIR_TY; t >= 8; t--) {   // marches shorter than 8 rows lost wherever they were tried
     const long long ctas = (long long)gx * ((C.ny + t - 1) / t);
-    if (t > 16 && ctas < slots) continue;
-    const long long cost = ((ctas + slots - 1) / slots) * (t + 5);
+    const long long cost = ((ctas + slots - 1) / slots) * (t + 6);
     if (best < 0 || cost < best) { best = cost; TY = t; }
   }
   // very small grids (less than four warps per SM even then): the march itself is what a launch-bound step waits for
