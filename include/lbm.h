@@ -113,6 +113,12 @@ typedef struct {
  * outside [0,180], mobility outside (0, 0.3), precision not 32/64, wall rows not solid). */
 int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_t* workspace_bytes);
 
+/* Relaxation time <-> kinematic viscosity of a phase, tau = 1/2 + nu / (c_s^2 dt) = 1/2 + 3 nu (dx = dt = 1,
+ * c_s^2 = 1/3): for callers who state the problem with tau per phase (north_star: "tau or viscosity per phase").
+ * Host arithmetic only. */
+double lbm_nu_from_tau(double tau);
+double lbm_tau_from_nu(double nu);
+
 /* Upper bound of the workspace size without touching a device or the mask (pure host arithmetic): what
  * lbm_create needs for a mask with at most `n_ghost_bound` ghost nodes in which every node group may hold
  * a fluid node.  lbm_plan's exact figure is never larger.  0 on bad parameters. */

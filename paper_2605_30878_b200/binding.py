@@ -24,7 +24,7 @@ SCHEDULE_INPLACE = 7
 FLUID_BULK, FLUID_BOUNDARY, GHOST, SOLID_BULK = 0, 1, 2, 3
 
 # include/lbm.h (the product boundary) and include/lbm_test.h (test and measurement hooks)
-EXPORTS = ("lbm_plan", "lbm_workspace_bytes", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
+EXPORTS = ("lbm_plan", "lbm_workspace_bytes", "lbm_nu_from_tau", "lbm_tau_from_nu", "lbm_create", "lbm_init", "lbm_step", "lbm_sync", "lbm_get",
            "lbm_get_populations", "lbm_set_populations", "lbm_rows_bytes", "lbm_rows_export", "lbm_rows_import",
            "lbm_keep_B", "lbm_sample_populations",
            "lbm_get_classification", "lbm_diag", "lbm_diag_static", "lbm_last_error", "lbm_version", "lbm_destroy")
@@ -106,6 +106,8 @@ def load_library() -> C.CDLL:
         L.lbm_plan.argtypes = [C.POINTER(_Params), vp, C.POINTER(i64), C.POINTER(C.c_size_t)]
         L.lbm_workspace_bytes.argtypes = [C.POINTER(_Params), i64]
         L.lbm_workspace_bytes.restype = C.c_size_t
+        for f in (L.lbm_nu_from_tau, L.lbm_tau_from_nu):
+            f.argtypes, f.restype = [C.c_double], C.c_double
         L.lbm_set_populations.argtypes = [vp, vp, vp]
         L.lbm_rows_bytes.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
         L.lbm_rows_export.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
@@ -150,6 +152,15 @@ def _f64(a, size=None):
     if size is not None and a.size != size:
         raise ValueError(f"expected {size} values, got {a.size}")
     return a
+
+
+def nu_from_tau(tau: float) -> float:
+    """Kinematic viscosity of a phase from its relaxation time (tau = 1/2 + 3 nu)."""
+    return float(load_library().lbm_nu_from_tau(float(tau)))
+
+
+def tau_from_nu(nu: float) -> float:
+    return float(load_library().lbm_tau_from_nu(float(nu)))
 
 
 def workspace_bytes(prm: LBMParams, n_ghost_bound: int) -> int:

@@ -647,6 +647,9 @@ int lbm_plan(const lbm_params* prm, const uint8_t* mask, int64_t* n_ghost, size_
   return LBM_OK;
 }
 
+double lbm_nu_from_tau(double tau) { return (tau - 0.5) / 3.0; }
+double lbm_tau_from_nu(double nu) { return 0.5 + 3.0 * nu; }
+
 size_t lbm_workspace_bytes(const lbm_params* prm, int64_t n_ghost_bound) {
   const char* why;
   if (validate(prm, &why) != LBM_OK || n_ghost_bound < 0) return 0;

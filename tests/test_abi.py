@@ -5,6 +5,7 @@ import os
 import re
 
 import numpy as np
+import pytest
 
 from paper_2605_30878_b200 import binding
 
@@ -84,3 +85,11 @@ def test_inplace_schedule_keeps_one_buffer_of_each_population_set():
         inpl = binding.workspace_bytes(binding.LBMParams(nx=nx, ny=ny, precision=prec, schedule=binding.SCHEDULE_INPLACE), 5000)
         saved = base - inpl
         assert 18 * nx * ny * rs <= saved <= 18 * (nx * ny + 4096) * rs + 18 * 256
+
+
+def test_tau_and_viscosity_helpers():
+    """tau = 1/2 + 3 nu; BASELINE config 1 states tau = 1 for both phases, i.e. nu = 1/6."""
+    assert binding.nu_from_tau(1.0) == pytest.approx(1.0 / 6.0, abs=1e-16)
+    assert binding.tau_from_nu(0.1) == pytest.approx(0.8, abs=1e-16)
+    for tau in (0.53, 0.8, 0.875, 1.0, 1.7):
+        assert binding.tau_from_nu(binding.nu_from_tau(tau)) == pytest.approx(tau, abs=1e-15)
